@@ -1,0 +1,203 @@
+// C-ABI boundary of the STARK decode library (declared in include/stark.h).
+// Argument validation first (no CUDA call), then dispatch to the launchers.
+#include <math.h>
+
+#include "common.cuh"
+
+namespace stark {
+
+int& last_cuda_error_ref() {
+    static int e = 0;
+    return e;
+}
+
+int num_sms() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
+            n = v;
+        else {
+            (void)cudaGetLastError();
+            return 148;  // B200; used for planning only
+        }
+    }
+    return n;
+}
+
+namespace {
+
+// 0 = unknown, 1 = sm_100, -1 = something else / no device
+int device_ok() {
+    static int state = 0;
+    if (state == 0) {
+        int dev = 0, major = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+            last_cuda_error_ref() = (int)cudaGetLastError();
+            return -2;
+        }
+        state = major == 10 ? 1 : -1;
+    }
+    return state;
+}
+
+int check_shape(const stark_shape_t* s) {
+    if (!s) return STARK_ERR_INVALID_ARG;
+    if (s->B < 1 || s->Hq < 1 || s->Hkv < 1 || s->D < 1 || s->d < 1 || s->Wmax < 1)
+        return STARK_ERR_INVALID_ARG;
+    if (s->Hq % s->Hkv != 0) return STARK_ERR_INVALID_ARG;
+    if (s->d > 8) return STARK_ERR_INVALID_ARG;
+    if (!(s->softmax_scale >= 0.f) || isinf(s->softmax_scale)) return STARK_ERR_INVALID_ARG;
+    if (s->dtype != STARK_F32 && s->dtype != STARK_BF16) return STARK_ERR_UNSUPPORTED;
+    if (s->D != 64 && s->D != 128) return STARK_ERR_UNSUPPORTED;
+    return STARK_OK;
+}
+
+int check_device() {
+    const int ok = device_ok();
+    if (ok == 1) return STARK_OK;
+    return ok == -2 ? STARK_ERR_CUDA : STARK_ERR_UNSUPPORTED;
+}
+
+int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+// Shape-only split choice.  Cost model: waves of CTAs x (KV tiles per CTA + a
+// fixed per-CTA overhead of ~1 tile); ties go to the smaller split count (less
+// partial traffic).
+int plan_splits(const Dims& p, int dtype, int n_q, int max_len) {
+    const int sms = num_sms();
+    const int tiles = ceil_div(max_len, 128);
+    const bool tc = prefix_tc_supported(p, dtype, n_q);
+    const long long M = (long long)n_q * p.G;
+    const long long base = (long long)p.B * p.Hkv * (tc ? ceil_div(M, 128) : ceil_div(M, 4));
+    const int per_sm = tc ? 1 : 4;  // resident CTAs per SM of each kernel
+    int best = 1;
+    double best_cost = 1e300;
+    for (int n = 1; n <= 64 && n <= tiles; ++n) {
+        const double waves = (double)ceil_div(base * n, (long long)sms * per_sm);
+        const double cost = waves * (ceil_div(tiles, n) + 1.0);
+        if (cost < best_cost * 0.97) { best_cost = cost; best = n; }
+    }
+    return best;
+}
+
+}  // namespace
+}  // namespace stark
+
+using namespace stark;
+
+extern "C" {
+
+int stark_version(void) { return STARK_VERSION; }
+
+const char* stark_status_string(int status) {
+    switch (status) {
+        case STARK_OK: return "STARK_OK";
+        case STARK_ERR_INVALID_ARG: return "STARK_ERR_INVALID_ARG: invalid argument";
+        case STARK_ERR_UNSUPPORTED: return "STARK_ERR_UNSUPPORTED: dtype, head_dim or device not supported";
+        case STARK_ERR_WORKSPACE: return "STARK_ERR_WORKSPACE: workspace missing or too small";
+        case STARK_ERR_CUDA: return "STARK_ERR_CUDA: a CUDA call failed (see stark_last_cuda_error)";
+        default: return "unknown stark status";
+    }
+}
+
+int stark_last_cuda_error(void) { return last_cuda_error_ref(); }
+
+size_t stark_suffix_bytes(const stark_shape_t* s) {
+    if (check_shape(s) != STARK_OK) return 0;
+    return (size_t)s->d * s->B * s->Wmax * s->Hkv * s->D * (s->dtype == STARK_F32 ? 4 : 2);
+}
+
+size_t stark_anc_bytes(const stark_shape_t* s) {
+    if (check_shape(s) != STARK_OK) return 0;
+    return (size_t)2 * s->B * s->Wmax * s->d * sizeof(int32_t);
+}
+
+size_t stark_workspace_bytes(const stark_shape_t* s, int call, int n_q, int total_tokens) {
+    if (!s) return 0;
+    if (call == STARK_CALL_BEAM_TOPK) {
+        if (s->B < 1 || n_q < 1 || total_tokens < 1) return 0;
+        return topk_workspace_bytes(s->B, n_q, total_tokens);
+    }
+    return 0;
+}
+
+int stark_prefix_attn_plan(const stark_shape_t* shape, int n_q, int total_tokens, int max_prefix_len,
+                           int* n_splits) {
+    int rc = check_shape(shape);
+    if (rc != STARK_OK) return rc;
+    if (!n_splits || n_q < 1 || total_tokens < 0 || max_prefix_len < 1) return STARK_ERR_INVALID_ARG;
+    *n_splits = plan_splits(make_dims(shape), shape->dtype, n_q, max_prefix_len);
+    return STARK_OK;
+}
+
+int stark_prefix_attn(const stark_shape_t* shape, const void* q, int n_q, const void* k_prefix,
+                      const void* v_prefix, const int32_t* cu_seqlens, int total_tokens,
+                      int max_prefix_len, int n_splits, float* part_m, float* part_l, float* part_o,
+                      void* ws, size_t ws_bytes, void* stream) {
+    (void)ws; (void)ws_bytes;
+    int rc = check_shape(shape);
+    if (rc != STARK_OK) return rc;
+    if (!q || !cu_seqlens || !part_m || !part_l || !part_o) return STARK_ERR_INVALID_ARG;
+    if (n_q < 1 || total_tokens < 0 || max_prefix_len < 1 || n_splits < 0 || n_splits > 64)
+        return STARK_ERR_INVALID_ARG;
+    if (total_tokens > 0 && (!k_prefix || !v_prefix)) return STARK_ERR_INVALID_ARG;
+    rc = check_device();
+    if (rc != STARK_OK) return rc;
+    const Dims p = make_dims(shape);
+    if (n_splits == 0) n_splits = plan_splits(p, shape->dtype, n_q, max_prefix_len);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (prefix_tc_supported(p, shape->dtype, n_q))
+        return launch_prefix_tc(p, q, n_q, k_prefix, v_prefix, cu_seqlens, total_tokens, n_splits, part_m,
+                                part_l, part_o, st);
+    return launch_prefix_simt(p, shape->dtype, q, n_q, k_prefix, v_prefix, cu_seqlens, n_splits, part_m,
+                              part_l, part_o, st);
+}
+
+int stark_tree_attn_step(const stark_shape_t* shape, const void* q, int n_q, int level,
+                         const void* k_suffix, const void* v_suffix, const int32_t* anc,
+                         const float* part_m, const float* part_l, const float* part_o, int n_splits,
+                         void* out, void* stream) {
+    int rc = check_shape(shape);
+    if (rc != STARK_OK) return rc;
+    if (!q || !part_m || !part_l || !part_o || !out) return STARK_ERR_INVALID_ARG;
+    if (n_q < 1 || n_splits < 1 || level < 0 || level > shape->d) return STARK_ERR_INVALID_ARG;
+    if (level >= 1 && (!k_suffix || !v_suffix || !anc || n_q > shape->Wmax)) return STARK_ERR_INVALID_ARG;
+    rc = check_device();
+    if (rc != STARK_OK) return rc;
+    return launch_tree_attn(make_dims(shape), shape->dtype, q, n_q, level, k_suffix, v_suffix, anc, part_m,
+                            part_l, part_o, n_splits, out, (cudaStream_t)stream);
+}
+
+int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_in, int C, int W_out,
+                    float* out_score, int32_t* out_parent, int32_t* out_code, void* ws, size_t ws_bytes,
+                    void* stream) {
+    if (!logp || !out_score || !out_parent || !out_code) return STARK_ERR_INVALID_ARG;
+    if (B < 1 || W_in < 1 || C < 1 || W_out < 1) return STARK_ERR_INVALID_ARG;
+    if ((long long)W_in * C >= (1ll << 31)) return STARK_ERR_INVALID_ARG;
+    if ((long long)W_out > (long long)W_in * C || W_out > 4096) return STARK_ERR_INVALID_ARG;
+    const size_t need = topk_workspace_bytes(B, W_in, C);
+    if (need > 0 && (!ws || ws_bytes < need)) return STARK_ERR_WORKSPACE;
+    int rc = check_device();
+    if (rc != STARK_OK) return rc;
+    return launch_topk(logp, score_or_null, B, W_in, C, W_out, out_score, out_parent, out_code, ws, ws_bytes,
+                       (cudaStream_t)stream);
+}
+
+int stark_kv_append_reorg(const stark_shape_t* shape, int level, int n_new, const void* k_new,
+                          const void* v_new, const int32_t* parent, void* k_suffix, void* v_suffix,
+                          int32_t* anc_or_null, void* stream) {
+    int rc = check_shape(shape);
+    if (rc != STARK_OK) return rc;
+    if (!k_new || !v_new || !k_suffix || !v_suffix) return STARK_ERR_INVALID_ARG;
+    if (level < 1 || level > shape->d || n_new < 1 || n_new > shape->Wmax) return STARK_ERR_INVALID_ARG;
+    if (level >= 2 && anc_or_null && !parent) return STARK_ERR_INVALID_ARG;
+    rc = check_device();
+    if (rc != STARK_OK) return rc;
+    return launch_append(make_dims(shape), shape->dtype, level, n_new, k_new, v_new, parent, k_suffix,
+                         v_suffix, anc_or_null, (cudaStream_t)stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,485 @@
+// A1 (tensor-core form): stark_prefix_attn for bf16 with M = n_q * G >= 64 rows
+// per (user, KV head) -- decode steps t >= 1.
+//
+// the conventional path recomputes attention over the shared
+// user-history prefix once per beam; STARK computes it once.  Here all
+// (beam, group-head) query rows of one (user, KV head) are packed into the M
+// dimension of a dense contraction against that user's prefix K/V tiles, so
+// each prefix byte is fetched once per step per M tile instead of once per
+// beam.  This is a real GEMM-shaped op (AI ~ M flop per KV byte), so it runs
+// on the 5th-generation tensor cores:
+//
+//   * one CTA per (M tile of 128 rows, KV head, split, user);
+//   * Q tile and K/V tiles staged in shared memory by TMA (cp.async.bulk.tensor,
+//     128-byte swizzle), K/V through an NS-stage mbarrier ring;
+//   * S = Q K^T by tcgen05.mma (SS, both operands K-major) into TMEM,
+//     double-buffered so that QK^T of tile j+1 overlaps the softmax of tile j;
+//   * softmax by 4 warps, one TMEM lane (= one query row) per thread: tcgen05.ld
+//     the S row, running reference maximum with lazy rescale (O is rescaled
+//     only when the row maximum grows by more than 2^8), exp2 in fp32, P packed
+//     to bf16 and written back to TMEM with tcgen05.st;
+//   * O += P V by tcgen05.mma with A = P from TMEM and B = V from shared
+//     memory (MN-major descriptor: V is [kv][D] with D contiguous);
+//   * epilogue: tcgen05.ld the O rows and emit the split-softmax partials
+//     (m, l, o) that stark_tree_attn_step merges by log-sum-exp.
+//
+// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator +
+// MMA issuer (one elected lane), warps 2..5 = softmax / correction / epilogue.
+// Every mbarrier wait is bounded (trap after ~1 s) so that a protocol bug
+// surfaces as a launch failure instead of a hung GPU.
+#include <cuda.h>
+
+#include "common.cuh"
+
+namespace stark {
+
+namespace {
+
+constexpr int BM = 128;          // query rows per CTA = MMA M
+constexpr int BN = 128;          // KV rows per tile   = MMA N of S, K-extent of P V
+constexpr int kThreadsTC = 192;
+constexpr int kSoftmaxThreads = 128;
+constexpr float kRescaleThreshold = 8.0f;  // log2 units
+
+// ---- PTX wrappers -------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    if (mbar_try(bar, parity)) return;
+    const long long t0 = clock64();
+    while (!mbar_try(bar, parity)) {
+        if (clock64() - t0 > (1ll << 31)) __trap();  // protocol bug: fail loudly, never hang
+    }
+}
+__device__ __forceinline__ void fence_barrier_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(dst), "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t addr, uint32_t ncols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]
+__device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc) : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem]
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(acc) : "memory");
+}
+
+// 32 consecutive fp32 columns of this thread's TMEM lane.
+__device__ __forceinline__ void tmem_ld32(uint32_t addr, uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(addr) : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t addr, const uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%32], "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31};"
+        ::"r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
+          "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
+          "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]),
+          "r"(addr) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ float fast_exp2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// ---- descriptors ----------------------------------------------------------------
+// Shared-memory matrix descriptor, 128-byte swizzle, descriptor version 1 (sm_100):
+//   [0,14) start>>4 | [16,30) leading byte offset>>4 | [32,46) stride byte offset>>4 |
+//   [46,48) version=1 | [61,64) layout=2 (SWIZZLE_128B)
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    return (uint64_t)((addr & 0x3ffffu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) |
+           ((uint64_t)(sbo_bytes >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+// Instruction descriptor, kind::f16: D=f32 [4,6)=1, A=bf16 [7,10)=1, B=bf16 [10,13)=1,
+// a_major bit 15, b_major bit 16 (0 = K-major, 1 = MN-major), N>>3 at [17,23), M>>4 at [24,29).
+__host__ __device__ constexpr uint32_t instr_desc(int M, int N, int b_mn_major) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(N >> 3) << 17) |
+           ((uint32_t)(M >> 4) << 24);
+}
+
+template <int D> struct TcCfg {
+    static constexpr int BOXES = D / 64;               // 64-element (128-byte) column boxes per row
+    static constexpr int TILE_BYTES = BOXES * BM * 128; // one 128-row tile of Q, K or V
+    static constexpr int NS = D == 128 ? 3 : 4;         // K/V pipeline depth
+    static constexpr int SMEM_BYTES = TILE_BYTES * (1 + 2 * NS) + 1024 /*align*/ + 256 /*barriers*/;
+    static constexpr int TMEM_COLS = 512;
+    static constexpr int COL_S = 0, COL_P = 256, COL_O = 384;
+};
+
+template <int D>
+__global__ void __launch_bounds__(kThreadsTC, 1)
+prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+                 const __grid_constant__ CUtensorMap tm_v, const int32_t* __restrict__ cu,
+                 float* __restrict__ pm, float* __restrict__ pl, float* __restrict__ po, int B, int n_q,
+                 int Hq, int Hkv, int G, int n_splits, float scale_log2) {
+    using C = TcCfg<D>;
+    constexpr int NS = C::NS;
+    const int mt = blockIdx.x;
+    const int kv = blockIdx.y % Hkv;
+    const int split = blockIdx.y / Hkv;
+    const int u = blockIdx.z;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    const int row_begin = cu[u];
+    const int L = cu[u + 1] - row_begin;
+    int chunk = (L + n_splits - 1) / n_splits;
+    chunk = ((chunk + 127) / 128) * 128;
+    const int r0 = split * chunk;
+    const int r1 = min(L, r0 + chunk);
+    const int n_tiles = r1 > r0 ? (r1 - r0 + BN - 1) / BN : 0;
+    const int beams_per_tile = BM / G;
+    const size_t split_stride = (size_t)B * n_q * Hq;
+
+    if (n_tiles == 0) {  // empty split: (m, l, o) = (-inf, 0, 0), reading R18
+        if (warp >= 2) {
+            const int r = threadIdx.x - 64;
+            const int i = mt * beams_per_tile + r / G, g = r % G;
+            if (i < n_q) {
+                const size_t row = split * split_stride + ((size_t)u * n_q + i) * Hq + kv * G + g;
+                pm[row] = -INFINITY; pl[row] = 0.f;
+                float4* o4 = reinterpret_cast<float4*>(po + row * D);
+                for (int c = 0; c < D / 4; ++c) o4[c] = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+        }
+        return;
+    }
+
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t sQ = smem_base;
+    const uint32_t sK = sQ + C::TILE_BYTES;
+    const uint32_t sV = sK + NS * C::TILE_BYTES;
+    const uint32_t sBar = sV + NS * C::TILE_BYTES;
+    // barrier slots (8 bytes each)
+    const uint32_t bar_q = sBar;
+    const uint32_t bar_kfull = sBar + 8;                 // [NS]
+    const uint32_t bar_kempty = bar_kfull + 8 * NS;      // [NS]
+    const uint32_t bar_vfull = bar_kempty + 8 * NS;      // [NS]
+    const uint32_t bar_vempty = bar_vfull + 8 * NS;      // [NS]
+    const uint32_t bar_sfull = bar_vempty + 8 * NS;      // [2]
+    const uint32_t bar_pfull = bar_sfull + 16;           // [2]
+    const uint32_t bar_pvdone = bar_pfull + 16;          // [2]
+    const uint32_t tmem_slot = bar_pvdone + 16;          // uint32
+    // generic pointer to the tmem slot
+    volatile uint32_t* tmem_slot_ptr =
+        reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    if (threadIdx.x == 0) {
+        mbar_init(bar_q, 1);
+        for (int s = 0; s < NS; ++s) {
+            mbar_init(bar_kfull + 8 * s, 1);
+            mbar_init(bar_kempty + 8 * s, 1);
+            mbar_init(bar_vfull + 8 * s, 1);
+            mbar_init(bar_vempty + 8 * s, 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar_sfull + 8 * b, 1);
+            mbar_init(bar_pfull + 8 * b, kSoftmaxThreads);
+            mbar_init(bar_pvdone + 8 * b, 1);
+        }
+        fence_barrier_init();
+    }
+    if (warp == 1) tmem_alloc(tmem_slot, C::TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        if (lane == 0) {
+            mbar_expect_tx(bar_q, C::TILE_BYTES);
+#pragma unroll
+            for (int bx = 0; bx < C::BOXES; ++bx)
+                tma_load_3d(sQ + bx * (BM * 128), &tm_q, bar_q, bx * 64, kv * G, u * n_q + mt * beams_per_tile);
+            for (int j = 0; j < n_tiles; ++j) {
+                const int s = j % NS;
+                const uint32_t ph = (uint32_t)((j / NS) & 1);
+                const int row = row_begin + r0 + j * BN;
+                mbar_wait(bar_kempty + 8 * s, ph ^ 1u);
+                mbar_expect_tx(bar_kfull + 8 * s, C::TILE_BYTES);
+#pragma unroll
+                for (int bx = 0; bx < C::BOXES; ++bx)
+                    tma_load_3d(sK + s * C::TILE_BYTES + bx * (BN * 128), &tm_k, bar_kfull + 8 * s, bx * 64, kv, row);
+                mbar_wait(bar_vempty + 8 * s, ph ^ 1u);
+                mbar_expect_tx(bar_vfull + 8 * s, C::TILE_BYTES);
+#pragma unroll
+                for (int bx = 0; bx < C::BOXES; ++bx)
+                    tma_load_3d(sV + s * C::TILE_BYTES + bx * (BN * 128), &tm_v, bar_vfull + 8 * s, bx * 64, kv, row);
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer =====================
+        if (lane == 0) {
+            constexpr uint32_t idesc_s = instr_desc(BM, BN, 0);
+            constexpr uint32_t idesc_o = instr_desc(BM, D, 1);
+            auto issue_qk = [&](int j) {
+                const int s = j % NS;
+                mbar_wait(bar_kfull + 8 * s, (uint32_t)((j / NS) & 1));
+                tc_fence_after();
+                const uint32_t d_tmem = tmem + C::COL_S + (j & 1) * BN;
+#pragma unroll
+                for (int k = 0; k < D / 16; ++k) {
+                    const uint32_t off = (k / 4) * (BM * 128) + (k % 4) * 32;  // box, then 32 B per K=16 step
+                    const uint64_t a = smem_desc(sQ + off, 16, 1024);
+                    const uint64_t b = smem_desc(sK + s * C::TILE_BYTES + off, 16, 1024);
+                    umma_ss(d_tmem, a, b, idesc_s, k > 0 ? 1u : 0u);
+                }
+                umma_commit(bar_sfull + 8 * (j & 1));
+                umma_commit(bar_kempty + 8 * s);
+            };
+            mbar_wait(bar_q, 0);
+            issue_qk(0);
+            for (int j = 0; j < n_tiles; ++j) {
+                if (j + 1 < n_tiles) issue_qk(j + 1);
+                const int s = j % NS;
+                mbar_wait(bar_vfull + 8 * s, (uint32_t)((j / NS) & 1));
+                mbar_wait(bar_pfull + 8 * (j & 1), (uint32_t)((j >> 1) & 1));
+                tc_fence_after();
+                const uint32_t a_tmem = tmem + C::COL_P + (j & 1) * (BN / 2);
+#pragma unroll
+                for (int k = 0; k < BN / 16; ++k) {
+                    // V tile: [kv row][64 d] boxes, MN-major B operand; 16 kv rows = 2048 B per K step
+                    const uint64_t b = smem_desc(sV + s * C::TILE_BYTES + k * 2048, BN * 128, 1024);
+                    umma_ts(tmem + C::COL_O, a_tmem + k * 8, b, idesc_o, (j > 0 || k > 0) ? 1u : 0u);
+                }
+                umma_commit(bar_vempty + 8 * s);
+                umma_commit(bar_pvdone + 8 * (j & 1));
+            }
+        }
+    } else {
+        // ===================== softmax / correction / epilogue =====================
+        const int quarter = warp & 3;                   // TMEM lane quarter this warp may access
+        const int r = quarter * 32 + lane;              // query row inside the M tile
+        const uint32_t lane_addr = tmem + ((uint32_t)(quarter * 32) << 16);
+        float m_ref = -INFINITY, l_sum = 0.f;
+        for (int j = 0; j < n_tiles; ++j) {
+            const int b = j & 1;
+            mbar_wait(bar_sfull + 8 * b, (uint32_t)((j >> 1) & 1));
+            __syncwarp();
+            tc_fence_after();
+            uint32_t sraw[4][32];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) tmem_ld32(lane_addr + C::COL_S + b * BN + c * 32, sraw[c]);
+            tmem_wait_ld();
+            const int valid = min(BN, r1 - (r0 + j * BN));  // columns of this tile inside the split
+            float tmax = -INFINITY;
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+#pragma unroll
+                for (int x = 0; x < 32; ++x) {
+                    float v = __uint_as_float(sraw[c][x]) * scale_log2;
+                    if (c * 32 + x >= valid) v = -INFINITY;
+                    sraw[c][x] = __float_as_uint(v);
+                    tmax = fmaxf(tmax, v);
+                }
+            // lazy rescale: keep the reference maximum unless the row maximum grew by > 2^8
+            bool grow = false;
+            float m_new = m_ref;
+            if (j == 0) {
+                m_new = tmax;
+            } else if (tmax > m_ref + kRescaleThreshold) {
+                m_new = tmax; grow = true;
+            }
+            if (__any_sync(0xffffffffu, grow)) {
+                // O holds the sum up to tile j-1: wait for that MMA, then scale this warp's rows
+                mbar_wait(bar_pvdone + 8 * ((j - 1) & 1), (uint32_t)(((j - 1) >> 1) & 1));
+                __syncwarp();
+                tc_fence_after();
+                const float alpha = grow ? fast_exp2(m_ref - m_new) : 1.0f;
+#pragma unroll
+                for (int c = 0; c < D / 32; ++c) {
+                    uint32_t o[32];
+                    tmem_ld32(lane_addr + C::COL_O + c * 32, o);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int x = 0; x < 32; ++x) o[x] = __float_as_uint(__uint_as_float(o[x]) * alpha);
+                    tmem_st32(lane_addr + C::COL_O + c * 32, o);
+                }
+                l_sum *= alpha;
+            }
+            m_ref = m_new;
+            // P = exp2(s - m_ref), packed to bf16x2 (element 2c in the low half)
+            uint32_t pk[2][32];
+            float psum = 0.f;
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+#pragma unroll
+                for (int x = 0; x < 32; x += 2) {
+                    const float p0 = fast_exp2(__uint_as_float(sraw[c][x]) - m_ref);
+                    const float p1 = fast_exp2(__uint_as_float(sraw[c][x + 1]) - m_ref);
+                    psum += p0 + p1;
+                    __nv_bfloat162 h = __floats2bfloat162_rn(p0, p1);
+                    pk[c >> 1][(c & 1) * 16 + (x >> 1)] = *reinterpret_cast<uint32_t*>(&h);
+                }
+            l_sum += psum;
+            // P buffer b was last read by the MMA of tile j-2
+            if (j >= 2) mbar_wait(bar_pvdone + 8 * b, (uint32_t)(((j - 2) >> 1) & 1));
+            __syncwarp();
+            tc_fence_after();
+            tmem_st32(lane_addr + C::COL_P + b * (BN / 2), pk[0]);
+            tmem_st32(lane_addr + C::COL_P + b * (BN / 2) + 32, pk[1]);
+            tmem_wait_st();
+            tc_fence_before();
+            mbar_arrive(bar_pfull + 8 * b);
+        }
+        // ---- epilogue: O row -> partials ----
+        mbar_wait(bar_pvdone + 8 * ((n_tiles - 1) & 1), (uint32_t)(((n_tiles - 1) >> 1) & 1));
+        __syncwarp();
+        tc_fence_after();
+        const int i = mt * beams_per_tile + r / G, g = r % G;
+        const bool live = i < n_q;
+        const size_t row = split * split_stride + ((size_t)u * n_q + (live ? i : 0)) * Hq + kv * G + g;
+        float4* o4 = reinterpret_cast<float4*>(po + row * D);
+#pragma unroll
+        for (int c = 0; c < D / 32; ++c) {
+            uint32_t o[32];
+            tmem_ld32(lane_addr + C::COL_O + c * 32, o);
+            tmem_wait_ld();
+            if (live) {
+#pragma unroll
+                for (int x = 0; x < 32; x += 4)
+                    o4[c * 8 + (x >> 2)] = make_float4(__uint_as_float(o[x]), __uint_as_float(o[x + 1]),
+                                                       __uint_as_float(o[x + 2]), __uint_as_float(o[x + 3]));
+            }
+        }
+        if (live) { pm[row] = m_ref * kLn2; pl[row] = l_sum; }
+        tc_fence_before();
+    }
+    __syncthreads();
+    if (warp == 1) {
+        __syncwarp();
+        tc_fence_after();
+        tmem_dealloc(tmem, C::TMEM_COLS);
+    }
+}
+
+// ---- host side ----------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        else
+            (void)cudaGetLastError();
+    }
+    return fn;
+}
+
+// bf16 tensor [n2][n1][D] (D contiguous, rows of n1*D), box = 64 x box1 x box2, 128-byte swizzle
+bool make_map(CUtensorMap* tm, const void* base, int D, int n1, long long n2, int box1, int box2) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return false;
+    cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)n1, (cuuint64_t)n2};
+    cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)n1 * D * 2};
+    cuuint32_t box[3] = {64, (cuuint32_t)box1, (cuuint32_t)box2};
+    cuuint32_t estr[3] = {1, 1, 1};
+    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int D>
+int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, int n_q,
+             const int32_t* cu, int n_splits, float* pm, float* pl, float* po, cudaStream_t st) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        STARK_CUDA_TRY(cudaFuncSetAttribute(prefix_tc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            TcCfg<D>::SMEM_BYTES));
+        attr_done = true;
+    }
+    const int M = n_q * p.G;
+    dim3 grid((M + BM - 1) / BM, p.Hkv * n_splits, p.B);
+    prefix_tc_kernel<D><<<grid, kThreadsTC, TcCfg<D>::SMEM_BYTES, st>>>(tq, tk, tv, cu, pm, pl, po, p.B, n_q, p.Hq,
+                                                                       p.Hkv, p.G, n_splits, p.scale * kLog2e);
+    STARK_LAUNCH_CHECK();
+    return STARK_OK;
+}
+
+}  // namespace
+
+bool prefix_tc_supported(const Dims& p, int dtype, int n_q) {
+    if (dtype != STARK_BF16) return false;
+    if (p.D != 64 && p.D != 128) return false;
+    if (p.G > BM || (BM % p.G) != 0) return false;
+    return (long long)n_q * p.G >= 64;
+}
+
+int launch_prefix_tc(const Dims& p, const void* q, int n_q, const void* k, const void* v, const int32_t* cu,
+                     int total_tokens, int n_splits, float* pm, float* pl, float* po, cudaStream_t st) {
+    if (total_tokens < 1)
+        return launch_prefix_simt(p, STARK_BF16, q, n_q, k, v, cu, n_splits, pm, pl, po, st);
+    CUtensorMap tq, tk, tv;
+    if (!make_map(&tq, q, p.D, p.Hq, (long long)p.B * n_q, p.G, BM / p.G) ||
+        !make_map(&tk, k, p.D, p.Hkv, total_tokens, 1, BN) || !make_map(&tv, v, p.D, p.Hkv, total_tokens, 1, BN)) {
+        last_cuda_error_ref() = (int)cudaErrorInvalidValue;
+        return STARK_ERR_CUDA;
+    }
+    if (p.D == 128) return launch_d<128>(p, tq, tk, tv, n_q, cu, n_splits, pm, pl, po, st);
+    return launch_d<64>(p, tq, tk, tv, n_q, cu, n_splits, pm, pl, po, st);
+}
+
+}  // namespace stark
