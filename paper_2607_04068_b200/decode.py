@@ -1,0 +1,70 @@
+"""One attention layer's STARK decode state: buffers + the order of the four calls.
+
+SURVEY.md section 3.2 / PAPER.md:263-286: per decode step t
+    stark_kv_append_reorg (t >= 1)  ->  stark_prefix_attn  ->  stark_tree_attn_step
+and, after the caller turned the attention output into log-probs,
+    stark_beam_topk.
+Only buffer ownership and call ordering live here; all arithmetic is in the library.
+"""
+from __future__ import annotations
+
+from typing import Optional, Sequence, Tuple
+
+import torch
+
+from . import binding as sb
+
+
+class StarkLayer:
+    """Prefix K/V (immutable, shared by all beams of a user), the compact
+    per-level suffix buffers and the ancestor index of ONE layer."""
+
+    def __init__(self, B: int, Hq: int, Hkv: int, D: int, d: int, Wmax: int, dtype: torch.dtype,
+                 k_prefix: torch.Tensor, v_prefix: torch.Tensor, cu_seqlens: torch.Tensor,
+                 max_prefix_len: int, softmax_scale: float = 0.0, n_q_per_step: Optional[Sequence[int]] = None):
+        self.shape = sb.make_shape(B, Hq, Hkv, D, d, Wmax, dtype, softmax_scale)
+        self.dtype, self.dev = dtype, k_prefix.device
+        self.k_prefix, self.v_prefix, self.cu = k_prefix, v_prefix, cu_seqlens
+        self.total_tokens = int(k_prefix.shape[0])
+        self.max_len = int(max_prefix_len)
+        self.k_suffix, self.v_suffix, self.anc = sb.alloc_suffix(self.shape, dtype, self.dev)
+        self._parts = {}
+        if n_q_per_step is not None:      # pre-allocate (CUDA-graph capture needs static buffers)
+            for n_q in set(n_q_per_step):
+                self._partials(n_q)
+
+    def _partials(self, n_q: int):
+        if n_q not in self._parts:
+            ns = sb.stark_prefix_attn_plan(self.shape, n_q, self.total_tokens, self.max_len)
+            self._parts[n_q] = (ns,) + sb.alloc_partials(self.shape, n_q, ns, self.dev)
+        return self._parts[n_q]
+
+    def append(self, level: int, k_new: torch.Tensor, v_new: torch.Tensor, parent: Optional[torch.Tensor],
+               write_anc: bool = True) -> None:
+        sb.stark_kv_append_reorg(self.shape, level, int(k_new.shape[1]), k_new, v_new, parent, self.k_suffix,
+                                 self.v_suffix, self.anc if write_anc else None)
+
+    def attend(self, level: int, q: torch.Tensor, out: Optional[torch.Tensor] = None,
+               anc: Optional[torch.Tensor] = None) -> torch.Tensor:
+        """Attention of the level-`level` queries q[B,n_q,Hq,D] over prefix + ancestor chain."""
+        n_q = int(q.shape[1])
+        ns, pm, pl, po = self._partials(n_q)
+        sb.stark_prefix_attn(self.shape, q, n_q, self.k_prefix, self.v_prefix, self.cu, self.total_tokens,
+                             self.max_len, ns, pm, pl, po)
+        if out is None:
+            out = torch.empty_like(q)
+        sb.stark_tree_attn_step(self.shape, q, n_q, level, self.k_suffix, self.v_suffix,
+                                self.anc if anc is None else anc, pm, pl, po, ns, out)
+        return out
+
+
+def beam_topk(logp: torch.Tensor, score: Optional[torch.Tensor], W_out: int,
+              out: Optional[Tuple[torch.Tensor, torch.Tensor, torch.Tensor]] = None):
+    """logp[B,W_in,C] fp32, score[B,W_in] fp32 or None -> (score, parent, code) [B,W_out]."""
+    B, W_in, C = logp.shape
+    if out is None:
+        out = (torch.empty((B, W_out), dtype=torch.float32, device=logp.device),
+               torch.empty((B, W_out), dtype=torch.int32, device=logp.device),
+               torch.empty((B, W_out), dtype=torch.int32, device=logp.device))
+    sb.stark_beam_topk(logp, score, B, W_in, C, W_out, out[0], out[1], out[2])
+    return out

@@ -1,0 +1,75 @@
+"""The C-ABI library loads, exports every symbol include/stark.h declares, and validates
+arguments before any CUDA call (no GPU needed)."""
+import ctypes
+import os
+import re
+
+import pytest
+import torch
+
+from paper_2607_04068_b200 import binding as sb
+from paper_2607_04068_b200.build import build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    build()
+    return sb.lib()
+
+
+def test_exports_match_header(L):
+    hdr = open(os.path.join(ROOT, "include", "stark.h")).read()
+    declared = set(re.findall(r"\b(stark_[a-z_]+)\s*\(", hdr))
+    assert declared == set(sb.EXPORTS), declared ^ set(sb.EXPORTS)
+    for name in declared:
+        assert hasattr(L, name), name
+    assert L.stark_version() == 100
+
+
+def test_status_strings(L):
+    for code in (0, -1, -2, -3, -4):
+        assert L.stark_status_string(code).decode().startswith("STARK_")
+    assert b"unknown" in L.stark_status_string(-99)
+
+
+def test_sizes(L):
+    sh = sb.make_shape(3, 8, 2, 64, 4, 10, torch.bfloat16)
+    assert L.stark_suffix_bytes(ctypes.byref(sh)) == 4 * 3 * 10 * 2 * 64 * 2
+    assert L.stark_anc_bytes(ctypes.byref(sh)) == 2 * 3 * 10 * 4 * 4
+    bad = sb.make_shape(3, 8, 3, 64, 4, 10, torch.bfloat16)     # Hq % Hkv != 0
+    assert L.stark_suffix_bytes(ctypes.byref(bad)) == 0
+
+
+def test_plan_is_deterministic_and_positive(L):
+    sh = sb.make_shape(16, 16, 4, 128, 3, 64, torch.bfloat16)
+    a = sb.stark_prefix_attn_plan(sh, 1, 16 * 1024, 1024)
+    b = sb.stark_prefix_attn_plan(sh, 1, 16 * 1024, 1024)
+    assert a == b and 1 <= a <= 64
+    assert 1 <= sb.stark_prefix_attn_plan(sh, 64, 16 * 1024, 1024) <= 64
+
+
+def test_validation_before_cuda(L):
+    sh = sb.make_shape(1, 4, 4, 64, 3, 8, torch.float32)
+    p = ctypes.c_void_p(16)     # non-null dummy, never dereferenced: validation fails first
+    assert L.stark_prefix_attn(ctypes.byref(sh), None, 1, p, p, p, 1, 1, 1, p, p, p, None, 0, None) == -1
+    assert L.stark_prefix_attn(ctypes.byref(sh), p, 0, p, p, p, 1, 1, 1, p, p, p, None, 0, None) == -1
+    assert L.stark_prefix_attn(ctypes.byref(sh), p, 1, p, p, p, 1, 1, 65, p, p, p, None, 0, None) == -1
+    bad_d = sb.make_shape(1, 4, 4, 96, 3, 8, torch.float32)
+    assert L.stark_prefix_attn(ctypes.byref(bad_d), p, 1, p, p, p, 1, 1, 1, p, p, p, None, 0, None) == -2
+    assert L.stark_tree_attn_step(ctypes.byref(sh), p, 1, 4, p, p, p, p, p, p, 1, p, None) == -1   # level > d
+    assert L.stark_tree_attn_step(ctypes.byref(sh), p, 9, 1, p, p, p, p, p, p, 1, p, None) == -1   # n_q > Wmax
+    assert L.stark_beam_topk(p, None, 1, 2, 4, 9, p, p, p, None, 0, None) == -1                    # W_out > W_in*C
+    assert L.stark_beam_topk(p, None, 1, 1 << 16, 1 << 16, 4, p, p, p, None, 0, None) == -1        # >= 2^31
+    assert L.stark_kv_append_reorg(ctypes.byref(sh), 0, 1, p, p, p, p, p, p, None) == -1           # level < 1
+    assert L.stark_kv_append_reorg(ctypes.byref(sh), 2, 1, p, p, None, p, p, p, None) == -1        # parent missing
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="only meaningful without a GPU")
+def test_no_cpu_fallback(L):
+    """Without a device a well-formed call fails loudly (never computes on the CPU)."""
+    sh = sb.make_shape(1, 4, 4, 64, 3, 8, torch.float32)
+    p = ctypes.c_void_p(16)
+    rc = L.stark_beam_topk(p, None, 1, 2, 4, 2, p, p, p, None, 0, None)
+    assert rc in (-2, -4)

@@ -1,0 +1,20 @@
+"""GPU parity: the CUDA path (through the C ABI) vs the fp64 oracle, teacher-forced
+on identical seeded inputs (SURVEY.md section 8(c) comparison protocol).
+Selection bit-exact; attention within 2e-3 (fp32) / 1.5e-2 (bf16) of max|out|."""
+import numpy as np
+import pytest
+
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+SMALL = ["cfg1", "f32_gqa", "cfg2_small", "cfg3_small", "cfg4_small", "cfg5_small", "paper_small"]
+
+
+@pytest.mark.parametrize("name", SMALL)
+def test_teacher_forced_parity(name):
+    from tests._parity import run_teacher_forced
+    rep = run_teacher_forced(wl.get_config(name))
+    bad = [r for r in rep if not r[2]]
+    assert not bad, f"{name}: {bad}\nfull report: {rep}"
+    assert any(r[0] == "topk" for r in rep) and any(r[0] == "attn" for r in rep)
