@@ -12,7 +12,7 @@ import torch
 
 import workloads as wl
 from oracle.beam_search import conventional_beam_search
-from oracle.token_models import DrawTokenModel
+from oracle.token_models import DrawTokenModel, TableTokenModel
 
 from paper_2607_04068_b200.decode import StarkLayer, beam_topk
 
@@ -33,6 +33,8 @@ def draws(cfg, seed=0, final_step=True):
     K, V, cu = wl.prefix_kv(cfg, seed)
     nq = wl.queries_per_step(cfg)
     steps = cfg.d + (1 if final_step else 0)
+    if cfg.logits == "projection":      # config 1: q/k/v/logits come from the token tables
+        return dict(K=K, V=V, cu=cu, tables=wl.config1_tables(cfg, seed), nq=nq, steps=steps)
     q, k, v, lg = [], [], [], []
     for t in range(steps):
         qq, kk, vv = wl.step_qkv(cfg, t, nq[t], seed)
@@ -47,8 +49,11 @@ def oracle_traces(cfg, dr, users=None, final_step=True):
     cu = dr["cu"]
     out = {}
     for u in (range(cfg.B) if users is None else users):
-        m = DrawTokenModel([x[u] for x in dr["q"]], [x[u] for x in dr["k"]], [x[u] for x in dr["v"]],
-                           [x[u] for x in dr["lg"]])
+        if "tables" in dr:
+            m = TableTokenModel(dr["tables"])
+        else:
+            m = DrawTokenModel([x[u] for x in dr["q"]], [x[u] for x in dr["k"]], [x[u] for x in dr["v"]],
+                               [x[u] for x in dr["lg"]])
         out[u] = conventional_beam_search(dr["K"][cu[u]:cu[u + 1]], dr["V"][cu[u]:cu[u + 1]], m, cfg.W, cfg.C,
                                           scale, final_step=final_step)
     return out
@@ -71,9 +76,12 @@ def run_teacher_forced(cfg, seed=0, final_step=True):
     report = []
     score = parent = None
     for t in range(dr["steps"]):
-        q = to_dev(dr["q"][t], dt)
+        # the oracle's trace holds the exact q / k_new / v_new it consumed (teacher forcing)
+        q = to_dev(np.stack([tr[u].q[t] for u in range(cfg.B)]).astype(np.float32), dt)
         if t >= 1:
-            layer.append(t, to_dev(dr["k"][t], dt), to_dev(dr["v"][t], dt), parent)
+            kn = np.stack([tr[u].k_new[t] for u in range(cfg.B)]).astype(np.float32)
+            vn = np.stack([tr[u].v_new[t] for u in range(cfg.B)]).astype(np.float32)
+            layer.append(t, to_dev(kn, dt), to_dev(vn, dt), parent)
         out = layer.attend(t, q).float().cpu().numpy().astype(np.float64)
         ref = np.stack([tr[u].attn_out[t] for u in range(cfg.B)])
         err = np.abs(out - ref).max() / np.abs(ref).max()

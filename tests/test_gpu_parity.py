@@ -13,7 +13,7 @@ SMALL = ["cfg1", "f32_gqa", "cfg2_small", "cfg3_small", "cfg4_small", "cfg5_smal
 
 @pytest.mark.parametrize("name", SMALL)
 def test_teacher_forced_parity(name):
-    from tests._parity import run_teacher_forced
+    from _parity import run_teacher_forced
     rep = run_teacher_forced(wl.get_config(name))
     bad = [r for r in rep if not r[2]]
     assert not bad, f"{name}: {bad}\nfull report: {rep}"
