@@ -1,0 +1,432 @@
+#!/usr/bin/env python
+"""bench.py -- STARK decode hot path on B200 (contract: see DESIGN.md section 7).
+
+A "step" = one whole pass of the hot path over one batch of
+BASELINE.json configs[1] ("cfg2"): decode steps t = 0,1,2, each
+    stark_kv_append_reorg (t>=1) -> stark_prefix_attn -> stark_tree_attn_step -> stark_beam_topk.
+metric = generated SIDs/s (B * W_d final beams per pass / pass time); also us per decode step.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl stark|reference] [--workload cfg2]
+
+N > 1 (torchrun): users are independent, so every rank runs its own batch (weak scaling, no data-path
+collective); time = max over ranks.  --impl reference times the CPU oracle (oracle/) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC, UNIT = "generated SIDs/s (tree-attn decode, all steps)", "SIDs/s"
+L2_BYTES = 126 * 2 ** 20
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--impl", default="stark", choices=["stark", "reference"])
+    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="launch eagerly instead of replaying CUDA graphs")
+    ap.add_argument("--sets", type=int, default=0, help="rotating input sets (0 = enough to exceed L2)")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {k: float(d[k]) for k in FALLBACK_PEAKS if k in d} | {"source": "measured"}
+    return dict(FALLBACK_PEAKS) | {"source": "fallback"}
+
+
+# ------------------------------------------------------------------------------------------
+# algorithmic work per launch
+def work_prefix(cfg, lens, n_q, n_splits):
+    eb, tot = cfg.elem_bytes, int(np.sum(lens))
+    flops = 4.0 * n_q * cfg.G * tot * cfg.D * cfg.Hkv
+    byts = 2.0 * cfg.D * eb * cfg.Hkv * tot + cfg.B * n_q * cfg.Hq * cfg.D * eb \
+        + n_splits * cfg.B * n_q * cfg.Hq * (cfg.D + 2) * 4
+    return flops, byts
+
+
+def work_tree(cfg, n_q, level, n_splits):
+    eb = cfg.elem_bytes
+    rows = cfg.B * n_q * cfg.Hq
+    return rows * cfg.D * eb * 2 + n_splits * rows * (cfg.D + 2) * 4 + cfg.B * n_q * cfg.Hkv * 2 * level * cfg.D * eb
+
+
+def work_topk(cfg, W_in, W_out):
+    return cfg.B * (W_in * cfg.C * 4 + W_in * 4 + W_out * 12)
+
+
+def work_append(cfg, n_new):
+    return cfg.B * n_new * (cfg.Hkv * 2 * 2 * cfg.D * cfg.elem_bytes + 8 * cfg.d)
+
+
+# ------------------------------------------------------------------------------------------
+def host_inputs(cfg, seed):
+    """Seeded synthetic inputs of one batch (numpy, host): DESIGN.md section 4 recipe."""
+    K, V, cu = wl.prefix_kv(cfg, seed)
+    nq = wl.queries_per_step(cfg)
+    q, k, v, lg = [], [], [], []
+    for t in range(cfg.d):
+        qq, kk, vv = wl.step_qkv(cfg, t, nq[t], seed)
+        q.append(qq), k.append(kk), v.append(vv)
+        lg.append(wl.step_logits(cfg, t, nq[t], seed))
+    return dict(K=K, V=V, cu=cu, q=q, k=k, v=v, lg=lg)
+
+
+def make_pass(cfg, h, dev):
+    import torch
+    from paper_2607_04068_b200.pipeline import DecodePass
+    dt = torch.float32 if cfg.dtype == "f32" else torch.bfloat16
+    up = lambda a, d=None: (torch.from_numpy(a).to(dev).to(d) if d is not None else torch.from_numpy(a).to(dev)).contiguous()
+    # log-softmax of the per-level logits is the caller's step before stark_beam_topk: untimed
+    logp = [torch.log_softmax(up(x), dim=-1).contiguous() for x in h["lg"]]
+    lens = np.diff(h["cu"])
+    return DecodePass(cfg.B, cfg.Hq, cfg.Hkv, cfg.D, cfg.d, cfg.C, wl.beam_widths(cfg), dt, up(h["K"], dt),
+                      up(h["V"], dt), up(h["cu"].astype(np.int32)), int(lens.max()), [up(x, dt) for x in h["q"]],
+                      [up(x, dt) for x in h["k"]], [up(x, dt) for x in h["v"]], logp)
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock + throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.samples, self.reasons, self.active, self.stop_flag, self.max_mhz = [], set(), False, False, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv, self.h = pynvml, pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception as e:  # noqa: BLE001
+            self.nv, self.err = None, repr(e)
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap"}
+        while not self.stop_flag:
+            try:
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                if self.active:
+                    self.samples.append(mhz)
+                    self.reasons |= {n for bit, n in names.items() if r & bit}
+            except Exception:  # noqa: BLE001
+                pass
+            time.sleep(0.002)
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def time_graph_loop(torch, fns, iters, use_graph=True):
+    """Average device time (us) of one call of each fn in `fns`, replayed round-robin `iters` times.
+    CUDA events on the launching stream; graphs remove the host launch gaps."""
+    if use_graph:
+        graphs = []
+        for f in fns:
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                f()
+            graphs.append(g)
+        calls = [g.replay for g in graphs]
+    else:
+        calls = fns
+    for i in range(min(3 * len(calls), iters)):
+        calls[i % len(calls)]()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for i in range(iters):
+        calls[i % len(calls)]()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) * 1e3 / iters
+
+
+# ------------------------------------------------------------------------------------------
+def oracle_sample(cfg, n_users, seed=0):
+    """The CPU oracle (conventional fp64 beam search, oracle/) as it stands on `n_users` users of the
+    workload.  Returns (seconds, SIDs generated, threads used)."""
+    from oracle.beam_search import conventional_beam_search
+    from oracle.token_models import DrawTokenModel
+    users = list(range(n_users))
+    lens = wl.prefix_lengths(cfg, seed)
+    nq = wl.queries_per_step(cfg)
+    per_user = []
+    for u in users:
+        K, V = wl.prefix_kv_user(cfg, u, int(lens[u]), seed)
+        q, k, v, lg = [], [], [], []
+        for t in range(cfg.d):
+            qq, kk, vv = wl.step_qkv(cfg, t, nq[t], seed, users=[u])
+            q.append(qq[0]), k.append(kk[0]), v.append(vv[0])
+            lg.append(wl.step_logits(cfg, t, nq[t], seed, users=[u])[0])
+        per_user.append((K, V, DrawTokenModel(q, k, v, lg)))
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+    except Exception:  # noqa: BLE001
+        threads = 1
+    t0 = time.perf_counter()
+    n_sids = 0
+    for K, V, m in per_user:
+        tr = conventional_beam_search(K, V, m, cfg.W, cfg.C, 1.0 / np.sqrt(cfg.D))
+        n_sids += tr.paths.shape[0]
+    return time.perf_counter() - t0, n_sids, threads
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_users = 1
+    for _ in range(args.warmup):
+        pass  # the oracle has no warm-up state; nothing to do
+    steps = max(1, min(args.steps, 5))
+    times, sids = [], 0
+    threads = 1
+    for _ in range(steps):
+        dt, n, threads = oracle_sample(cfg, n_users)
+        times.append(dt)
+        sids += n
+    total = float(np.sum(times))
+    val = sids / total
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / steps * cfg.B / n_users, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "sample": f"{n_users} of {cfg.B} users per step, all {cfg.d} decode steps"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle",
+                             "sample": f"{n_users} of {cfg.B} users x {steps} repeats"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------
+def run_stark(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_2607_04068_b200.build import build
+    from paper_2607_04068_b200 import binding as sb
+    from paper_2607_04068_b200.decode import beam_topk
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --impl stark needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    if rank == 0:
+        build()
+    if world > 1:
+        dist.barrier()
+    sb.lib()
+
+    # ---- inputs: R rotating sets so that consecutive passes never hit a warm L2 ----------------
+    h0 = host_inputs(cfg, seed=rank * 1000)
+    set_bytes = sum(a.nbytes // (2 if cfg.dtype == "bf16" else 1) for a in [h0["K"], h0["V"], *h0["q"], *h0["k"], *h0["v"]]) \
+        + sum(a.nbytes for a in h0["lg"])
+    R = args.sets or int(min(16, max(2, -(-2 * L2_BYTES // set_bytes))))
+    hosts = [h0] + [host_inputs(cfg, seed=rank * 1000 + r) for r in range(1, R)]
+    passes = [make_pass(cfg, h, dev) for h in hosts]
+    lens = np.diff(h0["cu"])
+    widths = wl.beam_widths(cfg)
+    nq = wl.queries_per_step(cfg)
+    sids_per_pass = cfg.B * widths[-1]
+    launches_per_pass = passes[0].launches
+
+    for p in passes:                       # eager warm-up: function attributes, lazy module load
+        p.run()
+    torch.cuda.synchronize()
+    use_graph = not args.no_graph
+    if use_graph:
+        calls = []
+        for p in passes:
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                p.run()
+            calls.append(g.replay)
+    else:
+        calls = [p.run for p in passes]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(max(3, args.warmup)):
+        calls[i % R]()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.active = True
+    e0.record()
+    for i in range(args.steps):
+        calls[i % R]()
+    e1.record()
+    barrier()
+    sampler.active = False
+    ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    if len(sampler.samples) < 5:           # short timed region: sample a longer replay of the same work
+        sampler.active = True
+        t_end = time.time() + 0.3
+        i = 0
+        while time.time() < t_end:
+            calls[i % R]()
+            i += 1
+            if i % 64 == 0:
+                torch.cuda.synchronize()
+        torch.cuda.synchronize()
+        sampler.active = False
+    sampler.stop_flag = True
+    ms_per_step = ms / args.steps
+    value = world * sids_per_pass / (ms_per_step * 1e-3)
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    # ---- per-kernel device times (graphs of single launches over the rotating sets) -------------
+    pk = peaks()
+    kern = {}
+    it = 40 * R
+    for t in range(cfg.d):
+        ns = passes[0].layer.n_splits(nq[t])
+        fl, by = work_prefix(cfg, lens, nq[t], ns)
+        us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.prefix(p.q[t])) for p in passes], it, use_graph)
+        kern[f"prefix_attn.t{t}"] = {"us": us, "bytes": by, "flops": fl, "n_splits": ns}
+        us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.tree(t, p.q[t], p.out[t])) for p in passes], it, use_graph)
+        kern[f"tree_attn_step.t{t}"] = {"us": us, "bytes": work_tree(cfg, nq[t], t, ns)}
+        w_in = nq[t]
+        us = time_graph_loop(torch, [(lambda p=p, t=t: beam_topk(p.logp[t], p.sel[t - 1][0] if t else None, widths[t],
+                                                                  out=p.sel[t])) for p in passes], it, use_graph)
+        kern[f"beam_topk.t{t}"] = {"us": us, "bytes": work_topk(cfg, w_in, widths[t])}
+        if t >= 1:
+            us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.append(t, p.k_new[t], p.v_new[t], p.sel[t - 1][1]))
+                                         for p in passes], it, use_graph)
+            kern[f"kv_append_reorg.t{t}"] = {"us": us, "bytes": work_append(cfg, nq[t])}
+    hbm, tfl = pk["hbm_gbs"], pk["bf16_tflops"]
+    for k, v in kern.items():
+        v["GBps"] = v["bytes"] / v["us"] * 1e-3
+        t_h = v["bytes"] / (hbm * 1e3)                       # us
+        t_t = v.get("flops", 0.0) / (tfl * 1e6) if cfg.dtype == "bf16" else 0.0
+        v["roofline_us"] = max(t_h, t_t)
+        v["bound"] = "tensor" if t_t > t_h else "hbm"
+        v["frac"] = v["roofline_us"] / v["us"]
+    ksum = sum(v["us"] for v in kern.values())
+    dom = max(kern, key=lambda k: kern[k]["us"])
+    dv = kern[dom]
+    if dv["bound"] == "tensor":
+        roof = {"bound": "tensor", "achieved": dv["flops"] / dv["us"] * 1e-6, "peak": tfl, "unit": "TFLOP/s"}
+    else:
+        roof = {"bound": "hbm", "achieved": dv["GBps"], "peak": hbm, "unit": "GB/s"}
+    roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": None, "kernel": dom,
+                 "kernel_us": dv["us"], "share_of_step": dv["us"] / ksum, "peak_source": pk["source"]})
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # written by hand from an ncu --set full capture
+    if os.path.exists(tpath):
+        roof["traffic"] = json.load(open(tpath)).get(cfg.name, {}).get(dom)
+
+    # ---- e2e: HOST buffers in, HOST result out, copies inside the timed region ------------------
+    p0, hst = passes[0], hosts[0]
+    dt_t = torch.float32 if cfg.dtype == "f32" else torch.bfloat16
+    pin = lambda a, d=None: (torch.from_numpy(a).to(d) if d is not None else torch.from_numpy(a)).contiguous().pin_memory()
+    src = [pin(hst["K"], dt_t), pin(hst["V"], dt_t), pin(hst["cu"].astype(np.int32))] \
+        + [pin(x, dt_t) for x in hst["q"]] + [pin(x, dt_t) for x in hst["k"]] + [pin(x, dt_t) for x in hst["v"]] \
+        + [x.cpu().pin_memory() for x in p0.logp]
+    dst = [p0.layer.k_prefix, p0.layer.v_prefix, p0.layer.cu] + p0.q + p0.k_new + p0.v_new + p0.logp
+    res_d = [x for s in p0.sel for x in s]
+    res_h = [torch.empty(x.shape, dtype=x.dtype).pin_memory() for x in res_d]
+    h2d = sum(x.numel() * x.element_size() for x in src)
+    d2h = sum(x.numel() * x.element_size() for x in res_h)
+
+    def e2e_step():
+        for s_, d_ in zip(src, dst):
+            d_.copy_(s_, non_blocking=True)
+        calls[0]()
+        for d_, h_ in zip(res_d, res_h):
+            h_.copy_(d_, non_blocking=True)
+        torch.cuda.current_stream().synchronize()        # the caller reads the result on the host
+
+    n_e2e = max(3, min(args.steps, 30))
+    for _ in range(3):
+        e2e_step()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(n_e2e):
+        e2e_step()
+    e1.record()
+    torch.cuda.synchronize()
+    e2e_ms = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3) / n_e2e
+    e2e = {"value": world * sids_per_pass / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": n_e2e,
+           "note": "prefix K/V + per-step q/k/v/log-probs copied from pinned host memory every pass; "
+                   "per-level (score,parent,code) read back"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
+            "config": {"workload": cfg.name, "B": cfg.B, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D,
+                       "prefix_len": [int(lens.min()), int(lens.max())], "beam": list(widths), "levels": cfg.d,
+                       "codebook": cfg.C, "decode_steps_per_pass": cfg.d,
+                       "l2": f"{R} rotating input sets ({R * set_bytes / 2**20:.0f} MiB > L2 126 MiB), no flush",
+                       "launch": "cuda_graph" if use_graph else "eager"},
+            "us_per_decode_step": ms_per_step * 1e3 / cfg.d,
+            "gpu_launches": launches_per_pass * args.steps,
+            "clocks": sampler.summary(), "e2e": e2e, "roofline": roof,
+            "kernels": {k: {a: (round(b, 4) if isinstance(b, float) else b) for a, b in v.items()} for k, v in kern.items()},
+            "kernel_sum_us": ksum}
+    if world == 1 and not args.no_cpu_baseline:
+        n_users = 8 if cfg.name == "cfg2" else 1
+        sec, n_sids, threads = oracle_sample(cfg, n_users)
+        line["cpu_baseline"] = {"value": n_sids / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "sample": f"{n_users} of {cfg.B} users of {cfg.name}, all {cfg.d} decode steps, "
+                                          f"{sec:.1f} s wall"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    cfg = wl.get_config(args.workload)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_stark(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -44,18 +44,31 @@ class StarkLayer:
         sb.stark_kv_append_reorg(self.shape, level, int(k_new.shape[1]), k_new, v_new, parent, self.k_suffix,
                                  self.v_suffix, self.anc if write_anc else None)
 
-    def attend(self, level: int, q: torch.Tensor, out: Optional[torch.Tensor] = None,
-               anc: Optional[torch.Tensor] = None) -> torch.Tensor:
-        """Attention of the level-`level` queries q[B,n_q,Hq,D] over prefix + ancestor chain."""
+    def prefix(self, q: torch.Tensor) -> None:
+        """A1: shared-prefix partials of q[B,n_q,Hq,D] into this layer's partial buffers."""
         n_q = int(q.shape[1])
         ns, pm, pl, po = self._partials(n_q)
         sb.stark_prefix_attn(self.shape, q, n_q, self.k_prefix, self.v_prefix, self.cu, self.total_tokens,
                              self.max_len, ns, pm, pl, po)
-        if out is None:
-            out = torch.empty_like(q)
+
+    def tree(self, level: int, q: torch.Tensor, out: torch.Tensor, anc: Optional[torch.Tensor] = None) -> None:
+        """A2: ancestor-chain attention + log-sum-exp merge with the partials written by prefix(q)."""
+        n_q = int(q.shape[1])
+        ns, pm, pl, po = self._partials(n_q)
         sb.stark_tree_attn_step(self.shape, q, n_q, level, self.k_suffix, self.v_suffix,
                                 self.anc if anc is None else anc, pm, pl, po, ns, out)
+
+    def attend(self, level: int, q: torch.Tensor, out: Optional[torch.Tensor] = None,
+               anc: Optional[torch.Tensor] = None) -> torch.Tensor:
+        """Attention of the level-`level` queries q[B,n_q,Hq,D] over prefix + ancestor chain."""
+        if out is None:
+            out = torch.empty_like(q)
+        self.prefix(q)
+        self.tree(level, q, out, anc)
         return out
+
+    def n_splits(self, n_q: int) -> int:
+        return self._partials(n_q)[0]
 
 
 def beam_topk(logp: torch.Tensor, score: Optional[torch.Tensor], W_out: int,

@@ -1,0 +1,60 @@
+"""One whole pass of the STARK hot path (all rows of SURVEY.md section 8(a)) for one batch:
+decode steps t = 0..d-1, each  append(t>=1) -> prefix_attn -> tree_attn_step -> beam_topk.
+
+Inputs (prefix K/V, per-step q / k_new / v_new, per-level log-probs) are device tensors;
+`DecodePass.run()` only enqueues library calls on the current stream, so a pass is CUDA-graph
+capturable (shapes are static per step).  The tree is data dependent: the
+parents chosen by stark_beam_topk at level t feed stark_kv_append_reorg at level t+1.
+"""
+from __future__ import annotations
+
+from typing import Dict, List, Optional
+
+import torch
+
+from .decode import StarkLayer, beam_topk
+
+
+class DecodePass:
+    def __init__(self, B: int, Hq: int, Hkv: int, D: int, d: int, C: int, widths: List[int], dtype: torch.dtype,
+                 k_prefix: torch.Tensor, v_prefix: torch.Tensor, cu_seqlens: torch.Tensor, max_prefix_len: int,
+                 q: List[torch.Tensor], k_new: List[torch.Tensor], v_new: List[torch.Tensor],
+                 logp: List[torch.Tensor]):
+        self.B, self.d, self.C, self.widths = B, d, C, list(widths)
+        self.n_q = [1] + self.widths                      # queries per user at step t
+        self.layer = StarkLayer(B, Hq, Hkv, D, d, max(self.widths), dtype, k_prefix, v_prefix, cu_seqlens,
+                                max_prefix_len, n_q_per_step=self.n_q[:d])
+        self.q, self.k_new, self.v_new, self.logp = q, k_new, v_new, logp
+        dev = k_prefix.device
+        self.out = [torch.empty_like(q[t]) for t in range(d)]
+        self.sel = [(torch.empty((B, w), dtype=torch.float32, device=dev),
+                     torch.empty((B, w), dtype=torch.int32, device=dev),
+                     torch.empty((B, w), dtype=torch.int32, device=dev)) for w in self.widths]
+
+    #: library kernels launched by one run(): step 0 = 3, steps >= 1 = 4 each
+    @property
+    def launches(self) -> int:
+        return 3 + 4 * (self.d - 1)
+
+    def run(self) -> None:
+        score = parent = None
+        for t in range(self.d):
+            if t >= 1:
+                self.layer.append(t, self.k_new[t], self.v_new[t], parent)
+            self.layer.attend(t, self.q[t], out=self.out[t])
+            score, parent, _ = beam_topk(self.logp[t], score, self.widths[t], out=self.sel[t])
+
+    def result(self) -> Dict[str, List[torch.Tensor]]:
+        return {"score": [s[0] for s in self.sel], "parent": [s[1] for s in self.sel],
+                "code": [s[2] for s in self.sel]}
+
+    def paths(self) -> torch.Tensor:
+        """[B, W_d, d] SID paths of the final beams in slot order (index bookkeeping for
+        reporting; not part of the timed path)."""
+        W = self.widths[-1]
+        slot = torch.arange(W, device=self.sel[-1][1].device).expand(self.B, W).long()
+        cols: List[Optional[torch.Tensor]] = [None] * self.d
+        for t in range(self.d - 1, -1, -1):
+            cols[t] = torch.gather(self.sel[t][2].long(), 1, slot)
+            slot = torch.gather(self.sel[t][1].long(), 1, slot)
+        return torch.stack(cols, dim=2)
