@@ -101,3 +101,76 @@ def run_teacher_forced(cfg, seed=0, final_step=True):
         if not ok:     # keep the tree identical to the oracle's for the later attention checks
             score, parent = to_dev(s_r), to_dev(p_r)
     return report
+
+
+# ---- full-size configs: the launch configuration bench.py times, sampled oracle checks -------------
+def run_full_size(cfg, n_samples=6, seed=0, use_graph=True):
+    """Free-running DecodePass (bench.py's own object, CUDA-graph replay) at BASELINE.json's full size.
+    Checks: (a) every level's selection, ALL users, bit-exact vs oracle.select_beams on the identical fp32
+    log-probs and scores; (b) the ancestor index vs oracle.ancestor_chains and the suffix K/V (bitwise copy);
+    (c) attention rows of sampled (user, beam) pairs vs oracle.replay_beam_attention (conventional
+    per-beam full-sequence attention, fp64); (d) the prefix buffers are bit-identical before/after."""
+    import bench
+    from oracle.selection import select_beams
+    from oracle.tree import ancestor_chains
+    from oracle.replay import replay_beam_attention
+    h = bench.host_inputs(cfg, seed)
+    p = bench.make_pass(cfg, h, torch.device("cuda"))
+    kp0, vp0 = p.layer.k_prefix.clone(), p.layer.v_prefix.clone()
+    p.run()
+    torch.cuda.synchronize()
+    if use_graph:
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            p.run()
+        for s in p.sel:                       # poison the outputs: the replay must rewrite them
+            s[1].fill_(-7)
+        g.replay()
+        torch.cuda.synchronize()
+    report = []
+    tol, scale = TOL[cfg.dtype], 1.0 / np.sqrt(cfg.D)
+    report.append(("prefix_untouched", -1, bool(torch.equal(kp0, p.layer.k_prefix) and torch.equal(vp0, p.layer.v_prefix)), ""))
+    logp = [x.cpu().numpy() for x in p.logp]
+    sel = [[x.cpu().numpy() for x in s] for s in p.sel]
+    rng = np.random.default_rng(1234 + cfg.config_id)
+    cu = h["cu"]
+    ks = p.layer.k_suffix.float().cpu().numpy()
+    vs = p.layer.v_suffix.float().cpu().numpy()
+    anc = p.layer.anc.cpu().numpy()
+    for t in range(cfg.d):
+        # (a) selection
+        ok = True
+        for u in range(cfg.B):
+            score = np.zeros(1, np.float32) if t == 0 else sel[t - 1][0][u]
+            s_r, p_r, c_r = select_beams(score, logp[t][u], p.widths[t])
+            ok &= (np.array_equal(sel[t][1][u], p_r) and np.array_equal(sel[t][2][u], c_r)
+                   and np.array_equal(sel[t][0][u].view(np.uint32), s_r.view(np.uint32)))
+        report.append(("topk_all_users", t, bool(ok), f"N={logp[t].shape[1] * cfg.C} W_out={p.widths[t]}"))
+        if t == 0:
+            pass
+        else:
+            # (b) append: K/V of level t are a bitwise copy; anc rows follow the parents
+            n = p.n_q[t]
+            ok_kv = np.array_equal(ks[t - 1][:, :n], h["k"][t]) and np.array_equal(vs[t - 1][:, :n], h["v"][t])
+            ok_anc = True
+            for u in range(cfg.B):
+                parents = [sel[l][1][u] for l in range(t)]
+                ok_anc &= np.array_equal(anc[t & 1, u, :n, :t], ancestor_chains(parents, t))
+            report.append(("append_kv_bitwise", t, bool(ok_kv), ""))
+            if t + 2 > cfg.d - 1:      # anc ping-pongs by level parity: level t's half is reused by level t+2
+                report.append(("anc_vs_oracle_chains", t, bool(ok_anc), ""))
+        # (c) sampled attention rows.  NOTE: after the whole pass anc/suffix hold the final state; level-t
+        # rows are never overwritten by later levels, so every step can be checked afterwards.
+        out = p.out[t].float().cpu().numpy().astype(np.float64)
+        worst, ref_max = 0.0, 0.0
+        for _ in range(n_samples):
+            u, i = int(rng.integers(cfg.B)), int(rng.integers(p.n_q[t]))
+            parents = [sel[l][1][u] for l in range(t)]
+            ref = replay_beam_attention(h["K"][cu[u]:cu[u + 1]], h["V"][cu[u]:cu[u + 1]],
+                                        [h["k"][l][u] for l in range(1, t + 1)], [h["v"][l][u] for l in range(1, t + 1)],
+                                        parents, h["q"][t][u, i], i, t, scale)
+            worst = max(worst, float(np.abs(out[u, i] - ref).max()))
+            ref_max = max(ref_max, float(np.abs(ref).max()))
+        report.append(("attn_sampled", t, bool(np.isfinite(out).all() and worst <= tol * ref_max),
+                       f"max_abs_err={worst:.3e} max|ref|={ref_max:.3e} tol={tol}"))
+    return report

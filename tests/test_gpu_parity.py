@@ -18,3 +18,13 @@ def test_teacher_forced_parity(name):
     bad = [r for r in rep if not r[2]]
     assert not bad, f"{name}: {bad}\nfull report: {rep}"
     assert any(r[0] == "topk" for r in rep) and any(r[0] == "attn" for r in rep)
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5"])
+def test_full_size_parity(name):
+    """BASELINE.json's full sizes in bench.py's launch configuration (DecodePass under CUDA-graph replay):
+    all selections bit-exact, append bitwise, sampled attention rows within tolerance."""
+    from _parity import run_full_size
+    rep = run_full_size(wl.get_config(name))
+    bad = [r for r in rep if not r[2]]
+    assert not bad, f"{name}: {bad}\nfull report: {rep}"
