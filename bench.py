@@ -143,28 +143,33 @@ class ClockSampler(threading.Thread):
 
 
 def time_graph_loop(torch, fns, iters, use_graph=True):
-    """Average device time (us) of one call of each fn in `fns`, replayed round-robin `iters` times.
-    CUDA events on the launching stream; graphs remove the host launch gaps."""
+    """Average device time (us) of one call of each fn in `fns` (one per rotating input set, so that
+    consecutive launches never find their inputs in L2).  All of them are captured, round-robin, into ONE
+    CUDA graph that is replayed; CUDA events on the launching stream bracket the replays.  (One graph per
+    launch would measure the graph-launch cadence instead: back-to-back single-kernel graphs start on a
+    ~2.05 us grid on this machine, see profiles/r01b_calibration.md.)"""
+    per_graph = max(len(fns), 24 // len(fns) * len(fns))
+    reps = max(1, iters // per_graph)
     if use_graph:
-        graphs = []
-        for f in fns:
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g):
-                f()
-            graphs.append(g)
-        calls = [g.replay for g in graphs]
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for i in range(per_graph):
+                fns[i % len(fns)]()
+        call = g.replay
     else:
-        calls = fns
-    for i in range(min(3 * len(calls), iters)):
-        calls[i % len(calls)]()
+        def call():
+            for i in range(per_graph):
+                fns[i % len(fns)]()
+    for _ in range(3):
+        call()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     e0.record()
-    for i in range(iters):
-        calls[i % len(calls)]()
+    for _ in range(reps):
+        call()
     e1.record()
     torch.cuda.synchronize()
-    return e0.elapsed_time(e1) * 1e3 / iters
+    return e0.elapsed_time(e1) * 1e3 / (reps * per_graph)
 
 
 # ------------------------------------------------------------------------------------------

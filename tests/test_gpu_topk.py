@@ -1,0 +1,85 @@
+"""GPU parity of stark_beam_topk (row A3) on adversarial inputs, bit-exact vs oracle.select_beams
+("adversarial exact ties, -inf blocks, W_out = W_in*C"; reading R6: key descending,
+flat index ascending, -0.0 == +0.0).  Every case exercises a different branch of the kernel: early exit after
+one radix pass, all three passes, the boundary-value tie path (ordered by index, across cluster ranks), the
+all-keys-equal shortcut, non-power-of-two codebooks, slices larger than the shared-memory cache."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def _check(logp, score, W_out):
+    import torch
+    from oracle.selection import select_beams
+    from paper_2607_04068_b200.decode import beam_topk
+    B, W_in, C = logp.shape
+    lp = torch.from_numpy(logp).cuda()
+    sc = None if score is None else torch.from_numpy(score).cuda()
+    s_g, p_g, c_g = [x.cpu().numpy() for x in beam_topk(lp, sc, W_out)]
+    for u in range(B):
+        s_r, p_r, c_r = select_beams(np.zeros(W_in, np.float32) if score is None else score[u], logp[u], W_out)
+        assert np.array_equal(p_g[u], p_r), f"user {u}: parent differs"
+        assert np.array_equal(c_g[u], c_r), f"user {u}: code differs"
+        assert np.array_equal(s_g[u].view(np.uint32), s_r.view(np.uint32)), f"user {u}: score bits differ"
+
+
+def _rng(tag):
+    return np.random.default_rng([0, 77, tag])
+
+
+@pytest.mark.parametrize("B,W_in,C,W_out", [
+    (3, 1, 32, 8), (2, 1, 256, 256), (5, 24, 48, 24), (2, 64, 256, 64), (2, 96, 160, 96),
+    (1, 512, 1024, 512), (3, 7, 33, 231), (2, 40, 97, 100), (1, 16, 8192, 512), (2, 130, 1000, 4096),
+])
+def test_random_logprobs(B, W_in, C, W_out):
+    r = _rng(1)
+    logits = r.normal(0, 2, (B, W_in, C))
+    logp = (logits - np.log(np.exp(logits).sum(-1, keepdims=True))).astype(np.float32)
+    score = None if W_in == 1 else np.sort(r.normal(-8, 2, (B, W_in)).astype(np.float32))[:, ::-1].copy()
+    _check(logp, score, W_out)
+
+
+@pytest.mark.parametrize("B,W_in,C,W_out", [(2, 64, 256, 64), (1, 512, 1024, 512), (3, 20, 50, 70)])
+def test_quantised_ties(B, W_in, C, W_out):
+    """Keys on a 1/8 grid: thousands of exact ties, the boundary value repeats far beyond the sort buffer."""
+    r = _rng(2)
+    logp = (np.round(r.normal(-6, 1.5, (B, W_in, C)) * 8) / 8).astype(np.float32)
+    score = (np.round(r.normal(-4, 1, (B, W_in)) * 8) / 8).astype(np.float32)
+    _check(logp, score, W_out)
+
+
+def test_all_equal_and_signed_zero():
+    logp = np.zeros((2, 16, 128), np.float32)
+    logp[0, ::2] = -0.0                      # -0.0 == +0.0: index order decides
+    _check(logp, None, 200)
+    _check(np.full((1, 64, 256), -3.25, np.float32), np.zeros((1, 64), np.float32), 64)
+    _check(np.full((2, 300, 512), -1.0, np.float32), None, 4096)
+
+
+def test_neg_inf_blocks():
+    r = _rng(3)
+    logp = r.normal(-5, 1, (2, 32, 256)).astype(np.float32)
+    logp[:, :, 10:] = -np.inf                # only 10 finite codes per beam: 320 finite keys
+    score = r.normal(-3, 1, (2, 32)).astype(np.float32)
+    _check(logp, score, 64)                  # all finite
+    _check(logp, score, 512)                 # 320 finite + 192 of the -inf keys, by index
+    logp[1] = -np.inf
+    _check(logp, score, 33)
+
+
+def test_two_values_boundary_inside_huge_tie():
+    """One distinct large key + a sea of equal keys: radix range is wide, boundary falls inside the tie."""
+    logp = np.full((2, 128, 512), -7.5, np.float32)
+    logp[0, 5, 17] = -0.125
+    logp[1, 127, 511] = -0.125
+    _check(logp, None, 300)
+
+
+def test_slice_larger_than_cache():
+    """B = 1, 2^20 candidates: slices exceed the shared-memory cache, later passes re-read through L2."""
+    r = _rng(4)
+    logp = r.normal(-9, 2, (1, 128, 8192)).astype(np.float32)
+    score = r.normal(-5, 1, (1, 128)).astype(np.float32)
+    _check(logp, score, 1024)
+    _check((np.round(logp * 4) / 4).astype(np.float32), (np.round(score * 4) / 4).astype(np.float32), 1024)
