@@ -64,20 +64,21 @@ int check_device() {
 int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 // Shape-only split choice.  Cost model: waves of CTAs x (KV tiles per CTA + a
-// fixed per-CTA overhead of ~1 tile); ties go to the smaller split count (less
-// partial traffic).
+// fixed per-CTA overhead of ~1 tile, ~2 for the tensor-core kernel whose
+// prologue allocates TMEM and fills the TMA ring); ties go to the smaller
+// split count (less partial traffic).
 int plan_splits(const Dims& p, int dtype, int n_q, int max_len) {
     const int sms = num_sms();
     const int tiles = ceil_div(max_len, 128);
     const bool tc = prefix_tc_supported(p, dtype, n_q);
     const long long M = (long long)n_q * p.G;
-    const long long base = (long long)p.B * p.Hkv * (tc ? ceil_div(M, 128) : ceil_div(M, 4));
+    const long long base = (long long)p.B * p.Hkv * (tc ? ceil_div(M, 256) : ceil_div(M, 4));  // CTAs per split
     const int per_sm = tc ? 1 : 4;  // resident CTAs per SM of each kernel
     int best = 1;
     double best_cost = 1e300;
     for (int n = 1; n <= 64 && n <= tiles; ++n) {
         const double waves = (double)ceil_div(base * n, (long long)sms * per_sm);
-        const double cost = waves * (ceil_div(tiles, n) + 1.0);
+        const double cost = waves * (ceil_div(tiles, n) + (tc ? 2.0 : 1.0));
         if (cost < best_cost * 0.97) { best_cost = cost; best = n; }
     }
     return best;

@@ -1,30 +1,39 @@
-// A1 (tensor-core form): stark_prefix_attn for bf16 with M = n_q * G >= 64 rows
-// per (user, KV head) -- decode steps t >= 1.
+// A1 (tensor-core form): stark_prefix_attn for bf16, any number of query rows.
 //
 // the conventional path recomputes attention over the shared
 // user-history prefix once per beam; STARK computes it once.  Here all
 // (beam, group-head) query rows of one (user, KV head) are packed into the M
 // dimension of a dense contraction against that user's prefix K/V tiles, so
-// each prefix byte is fetched once per step per M tile instead of once per
-// beam.  This is a real GEMM-shaped op (AI ~ M flop per KV byte), so it runs
-// on the 5th-generation tensor cores:
+// each prefix byte is fetched once per step per CTA instead of once per beam.
+// This is a real GEMM-shaped op (AI ~ M flop per KV byte), so it runs on the
+// 5th-generation tensor cores, organised like a two-tile flash-attention
+// forward whose epilogue emits split-softmax partials:
 //
-//   * one CTA per (M tile of 128 rows, KV head, split, user);
-//   * Q tile and K/V tiles staged in shared memory by TMA (cp.async.bulk.tensor,
-//     128-byte swizzle), K/V through an NS-stage mbarrier ring;
-//   * S = Q K^T by tcgen05.mma (SS, both operands K-major) into TMEM,
-//     double-buffered so that QK^T of tile j+1 overlaps the softmax of tile j;
-//   * softmax by 4 warps, one TMEM lane (= one query row) per thread: tcgen05.ld
-//     the S row, running reference maximum with lazy rescale (O is rescaled
-//     only when the row maximum grows by more than 2^8), exp2 in fp32, P packed
-//     to bf16 and written back to TMEM with tcgen05.st;
-//   * O += P V by tcgen05.mma with A = P from TMEM and B = V from shared
+//   * one CTA per (pair of 128-row Q tiles, KV head, prefix split, user): 256
+//     query rows share every K/V tile staged in shared memory;
+//   * Q tiles and K/V tiles arrive by TMA (cp.async.bulk.tensor, 128-byte
+//     swizzle); K and V alternate through one NS-slot mbarrier ring;
+//   * S_t = Q_t K^T by tcgen05.mma (SS, both operands K-major) into TMEM, one
+//     128-column accumulator per Q tile; P_t (bf16) overwrites S_t in place;
+//     O_t += P_t V by tcgen05.mma with A = P_t from TMEM and B = V from shared
 //     memory (MN-major descriptor: V is [kv][D] with D contiguous);
+//     TMEM columns: S0/P0 [0,128) S1/P1 [128,256) O0 [256,256+D) O1 [384,384+D);
+//   * two softmax warpgroups, one per Q tile, one TMEM lane (= query row) per
+//     thread.  The MMA warp issues  PV0_j, QK0_{j+1}, PV1_j, QK1_{j+1}, ...  so the
+//     tensor pipe works on one tile while the other tile's warpgroup runs its
+//     softmax (exp2 on the MUFU pipe) -- the two units stay busy together;
+//   * softmax streams its S row from TMEM twice (max, then exp2 + pack), 32
+//     columns at a time, so it needs few registers; running reference maximum
+//     with lazy rescale (O is touched only when a row maximum grows by > 2^8);
+//     the tensor pipe executes in issue order, so when S_t(j) is ready PV_t(j-1)
+//     has completed and O_t may be rescaled without another barrier;
 //   * epilogue: tcgen05.ld the O rows and emit the split-softmax partials
 //     (m, l, o) that stark_tree_attn_step merges by log-sum-exp.
 //
-// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator +
-// MMA issuer (one elected lane), warps 2..5 = softmax / correction / epilogue.
+// Decode step 0 (a single query per user, M = G rows) runs through the same
+// kernel: the contraction is then a pure HBM stream of the prefix (the tensor
+// pipe needs ~1/3 of the tile's HBM time), and warps without live rows skip
+// their softmax.
 // Every mbarrier wait is bounded (trap after ~1 s) so that a protocol bug
 // surfaces as a launch failure instead of a hung GPU.
 #include <cuda.h>
@@ -35,9 +44,9 @@ namespace stark {
 
 namespace {
 
-constexpr int BM = 128;          // query rows per CTA = MMA M
-constexpr int BN = 128;          // KV rows per tile   = MMA N of S, K-extent of P V
-constexpr int kThreadsTC = 192;
+constexpr int BM = 128;          // query rows per Q tile = MMA M (two Q tiles per CTA)
+constexpr int BN = 128;          // KV rows per tile      = MMA N of S, K-extent of P V
+constexpr int kThreadsTC = 320;  // TMA warp + MMA warp + 2 softmax warpgroups
 constexpr int kSoftmaxThreads = 128;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units
 
@@ -129,6 +138,15 @@ __device__ __forceinline__ void tmem_st32(uint32_t addr, const uint32_t (&r)[32]
           "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]),
           "r"(addr) : "memory");
 }
+// 16 consecutive 32-bit columns of this thread's TMEM lane.
+__device__ __forceinline__ void tmem_st16(uint32_t addr, const uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%16], "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15};"
+        ::"r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
+          "r"(addr) : "memory");
+}
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
@@ -153,13 +171,15 @@ __host__ __device__ constexpr uint32_t instr_desc(int M, int N, int b_mn_major) 
            ((uint32_t)(M >> 4) << 24);
 }
 
+
 template <int D> struct TcCfg {
-    static constexpr int BOXES = D / 64;               // 64-element (128-byte) column boxes per row
-    static constexpr int TILE_BYTES = BOXES * BM * 128; // one 128-row tile of Q, K or V
-    static constexpr int NS = D == 128 ? 3 : 4;         // K/V pipeline depth
-    static constexpr int SMEM_BYTES = TILE_BYTES * (1 + 2 * NS) + 1024 /*align*/ + 256 /*barriers*/;
+    static constexpr int BOXES = D / 64;                 // 64-element (128-byte) column boxes per row
+    static constexpr int TILE_BYTES = BOXES * BM * 128;  // one 128-row tile of Q, K or V
+    static constexpr int NS = D == 128 ? 5 : 8;          // K/V ring slots (K_j, V_j, K_j+1, ... in turn)
+    static constexpr int SMEM_BYTES = TILE_BYTES * (2 + NS) + 1024 /*align*/ + 256 /*barriers*/;
     static constexpr int TMEM_COLS = 512;
-    static constexpr int COL_S = 0, COL_P = 256, COL_O = 384;
+    static constexpr int COL_S = 0;                      // S_t / P_t at COL_S + t * 128
+    static constexpr int COL_O = 256;                    // O_t at COL_O + t * 128
 };
 
 template <int D>
@@ -170,7 +190,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                  int Hq, int Hkv, int G, int n_splits, float scale_log2) {
     using C = TcCfg<D>;
     constexpr int NS = C::NS;
-    const int mt = blockIdx.x;
+    const int pair = blockIdx.x;                         // Q tiles 2*pair and 2*pair + 1
     const int kv = blockIdx.y % Hkv;
     const int split = blockIdx.y / Hkv;
     const int u = blockIdx.z;
@@ -184,12 +204,15 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     const int r1 = min(L, r0 + chunk);
     const int n_tiles = r1 > r0 ? (r1 - r0 + BN - 1) / BN : 0;
     const int beams_per_tile = BM / G;
+    const int M = n_q * G;
+    const bool two = M > (2 * pair + 1) * BM;            // does the second Q tile hold any live row?
     const size_t split_stride = (size_t)B * n_q * Hq;
 
     if (n_tiles == 0) {  // empty split: (m, l, o) = (-inf, 0, 0), reading R18
         if (warp >= 2) {
-            const int r = threadIdx.x - 64;
-            const int i = mt * beams_per_tile + r / G, g = r % G;
+            const int t = (warp - 2) >> 2;
+            const int r = (threadIdx.x - 64) & 127;
+            const int i = (2 * pair + t) * beams_per_tile + r / G, g = r % G;
             if (i < n_q) {
                 const size_t row = split * split_stride + ((size_t)u * n_q + i) * Hq + kv * G + g;
                 pm[row] = -INFINITY; pl[row] = 0.f;
@@ -202,38 +225,50 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
 
     extern __shared__ unsigned char smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t sQ = smem_base;
-    const uint32_t sK = sQ + C::TILE_BYTES;
-    const uint32_t sV = sK + NS * C::TILE_BYTES;
-    const uint32_t sBar = sV + NS * C::TILE_BYTES;
+    const uint32_t sQ = smem_base;                       // Q0, Q1
+    const uint32_t sKV = sQ + 2 * C::TILE_BYTES;         // NS slots
+    const uint32_t sBar = sKV + NS * C::TILE_BYTES;
     // barrier slots (8 bytes each)
     const uint32_t bar_q = sBar;
-    const uint32_t bar_kfull = sBar + 8;                 // [NS]
-    const uint32_t bar_kempty = bar_kfull + 8 * NS;      // [NS]
-    const uint32_t bar_vfull = bar_kempty + 8 * NS;      // [NS]
-    const uint32_t bar_vempty = bar_vfull + 8 * NS;      // [NS]
-    const uint32_t bar_sfull = bar_vempty + 8 * NS;      // [2]
-    const uint32_t bar_pfull = bar_sfull + 16;           // [2]
-    const uint32_t bar_pvdone = bar_pfull + 16;          // [2]
-    const uint32_t tmem_slot = bar_pvdone + 16;          // uint32
-    // generic pointer to the tmem slot
+    const uint32_t bar_full = sBar + 8;                  // [NS] slot filled by TMA
+    const uint32_t bar_empty = bar_full + 8 * NS;        // [NS] slot consumed by the tensor pipe
+    const uint32_t bar_sfull = bar_empty + 8 * NS;       // [2]  S_t ready (and every earlier MMA done)
+    const uint32_t bar_pfull = bar_sfull + 16;           // [2]  P_t written by its warpgroup
+    const uint32_t bar_done = bar_pfull + 16;            // all MMAs of this CTA done
+    const uint32_t tmem_slot = bar_done + 8;             // uint32
     volatile uint32_t* tmem_slot_ptr =
         reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
+    // Warp 0 lane 0 initialises the barriers and immediately starts the first TMA loads: they only need
+    // the barriers, not TMEM, so the HBM latency of Q / K_0 / V_0 ... overlaps the TMEM allocation.
+    int n_issued = 0;
+    auto issue_kv = [&](int n) {                         // n = 2j: K_j, n = 2j + 1: V_j
+        const int s = n % NS;
+        const int row = row_begin + r0 + (n >> 1) * BN;
+        mbar_expect_tx(bar_full + 8 * s, C::TILE_BYTES);
+#pragma unroll
+        for (int bx = 0; bx < C::BOXES; ++bx)
+            tma_load_3d(sKV + s * C::TILE_BYTES + bx * (BN * 128), (n & 1) ? &tm_v : &tm_k, bar_full + 8 * s,
+                        bx * 64, kv, row);
+    };
     if (threadIdx.x == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_k) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_v) : "memory");
         mbar_init(bar_q, 1);
-        for (int s = 0; s < NS; ++s) {
-            mbar_init(bar_kfull + 8 * s, 1);
-            mbar_init(bar_kempty + 8 * s, 1);
-            mbar_init(bar_vfull + 8 * s, 1);
-            mbar_init(bar_vempty + 8 * s, 1);
-        }
-        for (int b = 0; b < 2; ++b) {
-            mbar_init(bar_sfull + 8 * b, 1);
-            mbar_init(bar_pfull + 8 * b, kSoftmaxThreads);
-            mbar_init(bar_pvdone + 8 * b, 1);
-        }
+        for (int s = 0; s < NS; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
+        for (int t = 0; t < 2; ++t) { mbar_init(bar_sfull + 8 * t, 1); mbar_init(bar_pfull + 8 * t, kSoftmaxThreads); }
+        mbar_init(bar_done, 1);
         fence_barrier_init();
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        const int beam0 = u * n_q + 2 * pair * beams_per_tile;
+        mbar_expect_tx(bar_q, (two ? 2 : 1) * C::TILE_BYTES);
+        for (int t = 0; t < (two ? 2 : 1); ++t)
+#pragma unroll
+            for (int bx = 0; bx < C::BOXES; ++bx)
+                tma_load_3d(sQ + t * C::TILE_BYTES + bx * (BM * 128), &tm_q, bar_q, bx * 64, kv * G,
+                            beam0 + t * beams_per_tile);
+        for (; n_issued < min(NS, 2 * n_tiles); ++n_issued) issue_kv(n_issued);  // the ring starts empty
     }
     if (warp == 1) tmem_alloc(tmem_slot, C::TMEM_COLS);
     tc_fence_before();
@@ -242,26 +277,11 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     const uint32_t tmem = *tmem_slot_ptr;
 
     if (warp == 0) {
-        // ===================== TMA producer =====================
+        // ===================== TMA producer (rest of the stream) =====================
         if (lane == 0) {
-            mbar_expect_tx(bar_q, C::TILE_BYTES);
-#pragma unroll
-            for (int bx = 0; bx < C::BOXES; ++bx)
-                tma_load_3d(sQ + bx * (BM * 128), &tm_q, bar_q, bx * 64, kv * G, u * n_q + mt * beams_per_tile);
-            for (int j = 0; j < n_tiles; ++j) {
-                const int s = j % NS;
-                const uint32_t ph = (uint32_t)((j / NS) & 1);
-                const int row = row_begin + r0 + j * BN;
-                mbar_wait(bar_kempty + 8 * s, ph ^ 1u);
-                mbar_expect_tx(bar_kfull + 8 * s, C::TILE_BYTES);
-#pragma unroll
-                for (int bx = 0; bx < C::BOXES; ++bx)
-                    tma_load_3d(sK + s * C::TILE_BYTES + bx * (BN * 128), &tm_k, bar_kfull + 8 * s, bx * 64, kv, row);
-                mbar_wait(bar_vempty + 8 * s, ph ^ 1u);
-                mbar_expect_tx(bar_vfull + 8 * s, C::TILE_BYTES);
-#pragma unroll
-                for (int bx = 0; bx < C::BOXES; ++bx)
-                    tma_load_3d(sV + s * C::TILE_BYTES + bx * (BN * 128), &tm_v, bar_vfull + 8 * s, bx * 64, kv, row);
+            for (int n = n_issued; n < 2 * n_tiles; ++n) {
+                mbar_wait(bar_empty + 8 * (n % NS), (uint32_t)(((n / NS) & 1) ^ 1));
+                issue_kv(n);
             }
         }
     } else if (warp == 1) {
@@ -269,138 +289,168 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
         if (lane == 0) {
             constexpr uint32_t idesc_s = instr_desc(BM, BN, 0);
             constexpr uint32_t idesc_o = instr_desc(BM, D, 1);
-            auto issue_qk = [&](int j) {
-                const int s = j % NS;
-                mbar_wait(bar_kfull + 8 * s, (uint32_t)((j / NS) & 1));
-                tc_fence_after();
-                const uint32_t d_tmem = tmem + C::COL_S + (j & 1) * BN;
+            // S_t = Q_t K_j^T; K_j sits in ring slot s
+            auto issue_qk = [&](int t, int s) {
+                const uint32_t d_tmem = tmem + C::COL_S + t * BN;
 #pragma unroll
                 for (int k = 0; k < D / 16; ++k) {
                     const uint32_t off = (k / 4) * (BM * 128) + (k % 4) * 32;  // box, then 32 B per K=16 step
-                    const uint64_t a = smem_desc(sQ + off, 16, 1024);
-                    const uint64_t b = smem_desc(sK + s * C::TILE_BYTES + off, 16, 1024);
-                    umma_ss(d_tmem, a, b, idesc_s, k > 0 ? 1u : 0u);
+                    umma_ss(d_tmem, smem_desc(sQ + t * C::TILE_BYTES + off, 16, 1024),
+                            smem_desc(sKV + s * C::TILE_BYTES + off, 16, 1024), idesc_s, k > 0 ? 1u : 0u);
                 }
-                umma_commit(bar_sfull + 8 * (j & 1));
-                umma_commit(bar_kempty + 8 * s);
+                umma_commit(bar_sfull + 8 * t);
             };
-            mbar_wait(bar_q, 0);
-            issue_qk(0);
-            for (int j = 0; j < n_tiles; ++j) {
-                if (j + 1 < n_tiles) issue_qk(j + 1);
-                const int s = j % NS;
-                mbar_wait(bar_vfull + 8 * s, (uint32_t)((j / NS) & 1));
-                mbar_wait(bar_pfull + 8 * (j & 1), (uint32_t)((j >> 1) & 1));
-                tc_fence_after();
-                const uint32_t a_tmem = tmem + C::COL_P + (j & 1) * (BN / 2);
+            // O_t (+)= P_t V_j; V tile: [kv row][64 d] boxes, MN-major B operand; 16 kv rows = 2048 B per K step
+            auto issue_pv = [&](int t, int s, bool acc) {
 #pragma unroll
-                for (int k = 0; k < BN / 16; ++k) {
-                    // V tile: [kv row][64 d] boxes, MN-major B operand; 16 kv rows = 2048 B per K step
-                    const uint64_t b = smem_desc(sV + s * C::TILE_BYTES + k * 2048, BN * 128, 1024);
-                    umma_ts(tmem + C::COL_O, a_tmem + k * 8, b, idesc_o, (j > 0 || k > 0) ? 1u : 0u);
+                for (int k = 0; k < BN / 16; ++k)
+                    umma_ts(tmem + C::COL_O + t * 128, tmem + C::COL_S + t * BN + k * 8,
+                            smem_desc(sKV + s * C::TILE_BYTES + k * 2048, BN * 128, 1024), idesc_o,
+                            (acc || k > 0) ? 1u : 0u);
+            };
+            auto slot_of = [&](int n) { return n % NS; };
+            auto wait_full = [&](int n) { mbar_wait(bar_full + 8 * slot_of(n), (uint32_t)((n / NS) & 1)); tc_fence_after(); };
+            const int nt = two ? 2 : 1;
+            mbar_wait(bar_q, 0);
+            wait_full(0);
+            for (int t = 0; t < nt; ++t) issue_qk(t, slot_of(0));
+            umma_commit(bar_empty + 8 * slot_of(0));
+            for (int j = 0; j < n_tiles; ++j) {
+                const bool more = j + 1 < n_tiles;
+                wait_full(2 * j + 1);                    // V_j
+                if (more) wait_full(2 * j + 2);          // K_{j+1}
+                for (int t = 0; t < nt; ++t) {
+                    mbar_wait(bar_pfull + 8 * t, (uint32_t)(j & 1));
+                    tc_fence_after();
+                    issue_pv(t, slot_of(2 * j + 1), j > 0);
+                    if (more) issue_qk(t, slot_of(2 * j + 2));
                 }
-                umma_commit(bar_vempty + 8 * s);
-                umma_commit(bar_pvdone + 8 * (j & 1));
+                umma_commit(bar_empty + 8 * slot_of(2 * j + 1));
+                if (more) umma_commit(bar_empty + 8 * slot_of(2 * j + 2));
             }
+            umma_commit(bar_done);
         }
     } else {
         // ===================== softmax / correction / epilogue =====================
+        const int t = (warp - 2) >> 2;                  // Q tile (= warpgroup) of this warp
         const int quarter = warp & 3;                   // TMEM lane quarter this warp may access
-        const int r = quarter * 32 + lane;              // query row inside the M tile
-        const uint32_t lane_addr = tmem + ((uint32_t)(quarter * 32) << 16);
-        float m_ref = -INFINITY, l_sum = 0.f;
-        for (int j = 0; j < n_tiles; ++j) {
-            const int b = j & 1;
-            mbar_wait(bar_sfull + 8 * b, (uint32_t)((j >> 1) & 1));
-            __syncwarp();
-            tc_fence_after();
-            uint32_t sraw[4][32];
-#pragma unroll
-            for (int c = 0; c < 4; ++c) tmem_ld32(lane_addr + C::COL_S + b * BN + c * 32, sraw[c]);
-            tmem_wait_ld();
-            const int valid = min(BN, r1 - (r0 + j * BN));  // columns of this tile inside the split
-            float tmax = -INFINITY;
-#pragma unroll
-            for (int c = 0; c < 4; ++c)
-#pragma unroll
-                for (int x = 0; x < 32; ++x) {
-                    float v = __uint_as_float(sraw[c][x]) * scale_log2;
-                    if (c * 32 + x >= valid) v = -INFINITY;
-                    sraw[c][x] = __float_as_uint(v);
-                    tmax = fmaxf(tmax, v);
-                }
-            // lazy rescale: keep the reference maximum unless the row maximum grew by > 2^8
-            bool grow = false;
-            float m_new = m_ref;
-            if (j == 0) {
-                m_new = tmax;
-            } else if (tmax > m_ref + kRescaleThreshold) {
-                m_new = tmax; grow = true;
-            }
-            if (__any_sync(0xffffffffu, grow)) {
-                // O holds the sum up to tile j-1: wait for that MMA, then scale this warp's rows
-                mbar_wait(bar_pvdone + 8 * ((j - 1) & 1), (uint32_t)(((j - 1) >> 1) & 1));
+        const int r = quarter * 32 + lane;              // query row inside the Q tile
+        const int i = (2 * pair + t) * beams_per_tile + r / G, g = r % G;
+        const bool live = i < n_q;
+        const bool warp_live = __any_sync(0xffffffffu, live);
+        if (t == 0 || two) {
+            const uint32_t lane_addr = tmem + ((uint32_t)(quarter * 32) << 16);
+            const uint32_t aS = lane_addr + C::COL_S + t * BN, aO = lane_addr + C::COL_O + t * 128;
+            float m_ref = -INFINITY, l_sum = 0.f;       // m_ref in log2 units of the scaled score
+            for (int j = 0; j < n_tiles; ++j) {
+                mbar_wait(bar_sfull + 8 * t, (uint32_t)(j & 1));
                 __syncwarp();
+                if (warp_live) {                        // warps without live rows only keep the barrier count
+                    tc_fence_after();
+                    const int valid = min(BN, r1 - (r0 + j * BN));  // columns of this tile inside the split
+                    // pass 1 over the S row: maximum
+                    float tmax = -INFINITY;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        uint32_t sr[32];
+                        tmem_ld32(aS + c * 32, sr);
+                        tmem_wait_ld();
+                        if (valid >= BN) {
+#pragma unroll
+                            for (int x = 0; x < 32; ++x) tmax = fmaxf(tmax, __uint_as_float(sr[x]));
+                        } else {
+#pragma unroll
+                            for (int x = 0; x < 32; ++x)
+                                if (c * 32 + x < valid) tmax = fmaxf(tmax, __uint_as_float(sr[x]));
+                        }
+                    }
+                    tmax *= scale_log2;
+                    // lazy rescale: keep the reference maximum unless the row maximum grew by > 2^8
+                    bool grow = false;
+                    float m_new = m_ref;
+                    if (j == 0) m_new = tmax;
+                    else if (tmax > m_ref + kRescaleThreshold) { m_new = tmax; grow = true; }
+                    if (__any_sync(0xffffffffu, grow)) {
+                        // S_t(j) ready => PV_t(j-1) completed (in-order tensor pipe): O_t is quiescent
+                        const float alpha = grow ? fast_exp2(m_ref - m_new) : 1.0f;
+#pragma unroll
+                        for (int c = 0; c < D / 32; ++c) {
+                            uint32_t o[32];
+                            tmem_ld32(aO + c * 32, o);
+                            tmem_wait_ld();
+#pragma unroll
+                            for (int x = 0; x < 32; ++x) o[x] = __float_as_uint(__uint_as_float(o[x]) * alpha);
+                            tmem_st32(aO + c * 32, o);
+                        }
+                        l_sum *= alpha;
+                    }
+                    m_ref = m_new;
+                    // pass 2: P = exp2(s * scale - m_ref) as bf16, written over S in place (P chunk c covers
+                    // columns [16c, 16c+16), all of them already consumed)
+                    const float neg_m = -m_ref;
+                    float psum = 0.f;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        uint32_t sr[32], pk[16];
+                        tmem_ld32(aS + c * 32, sr);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int x = 0; x < 32; x += 2) {
+                            float p0 = fast_exp2(fmaf(__uint_as_float(sr[x]), scale_log2, neg_m));
+                            float p1 = fast_exp2(fmaf(__uint_as_float(sr[x + 1]), scale_log2, neg_m));
+                            if (valid < BN) {
+                                if (c * 32 + x >= valid) p0 = 0.f;
+                                if (c * 32 + x + 1 >= valid) p1 = 0.f;
+                            }
+                            psum += p0 + p1;
+                            const __nv_bfloat162 h = __floats2bfloat162_rn(p0, p1);  // element 2x in the low half
+                            pk[x >> 1] = *reinterpret_cast<const uint32_t*>(&h);
+                        }
+                        tmem_st16(aS + c * 16, pk);
+                    }
+                    l_sum += psum;
+                    tmem_wait_st();
+                    tc_fence_before();
+                }
+                mbar_arrive(bar_pfull + 8 * t);
+            }
+            // ---- epilogue: O row -> partials ----
+            mbar_wait(bar_done, 0);
+            __syncwarp();
+            if (warp_live) {
                 tc_fence_after();
-                const float alpha = grow ? fast_exp2(m_ref - m_new) : 1.0f;
+                // Each thread owns one O row (512 B), so direct stores would scatter 16-byte pieces over 32
+                // rows per instruction (measured: 5.5 us for 17 MB).  Stage the warp's 32 rows in the (now
+                // idle) K/V ring, 16-byte chunks XOR-swizzled by row, then write whole rows coalesced.
+                constexpr int CPR = D / 4;              // 16-byte chunks per row
+                float* stage = reinterpret_cast<float*>(smem_raw + (sKV - smem_u32(smem_raw))) + (size_t)(warp - 2) * 32 * D;
 #pragma unroll
                 for (int c = 0; c < D / 32; ++c) {
                     uint32_t o[32];
-                    tmem_ld32(lane_addr + C::COL_O + c * 32, o);
+                    tmem_ld32(aO + c * 32, o);
                     tmem_wait_ld();
 #pragma unroll
-                    for (int x = 0; x < 32; ++x) o[x] = __float_as_uint(__uint_as_float(o[x]) * alpha);
-                    tmem_st32(lane_addr + C::COL_O + c * 32, o);
+                    for (int x = 0; x < 32; x += 4) {
+                        const int ch = (c * 8 + (x >> 2)) ^ (lane & (CPR - 1));
+                        *reinterpret_cast<float4*>(stage + lane * D + ch * 4) =
+                            make_float4(__uint_as_float(o[x]), __uint_as_float(o[x + 1]), __uint_as_float(o[x + 2]),
+                                        __uint_as_float(o[x + 3]));
+                    }
                 }
-                l_sum *= alpha;
-            }
-            m_ref = m_new;
-            // P = exp2(s - m_ref), packed to bf16x2 (element 2c in the low half)
-            uint32_t pk[2][32];
-            float psum = 0.f;
-#pragma unroll
-            for (int c = 0; c < 4; ++c)
-#pragma unroll
-                for (int x = 0; x < 32; x += 2) {
-                    const float p0 = fast_exp2(__uint_as_float(sraw[c][x]) - m_ref);
-                    const float p1 = fast_exp2(__uint_as_float(sraw[c][x + 1]) - m_ref);
-                    psum += p0 + p1;
-                    __nv_bfloat162 h = __floats2bfloat162_rn(p0, p1);
-                    pk[c >> 1][(c & 1) * 16 + (x >> 1)] = *reinterpret_cast<uint32_t*>(&h);
+                const size_t row_base = split * split_stride + (size_t)u * n_q * Hq + kv * G;
+                if (live) { pm[row_base + (size_t)i * Hq + g] = m_ref * kLn2; pl[row_base + (size_t)i * Hq + g] = l_sum; }
+                __syncwarp();
+                for (int idx = lane; idx < 32 * CPR; idx += 32) {
+                    const int l2 = idx / CPR, ch = idx % CPR;
+                    const int r2 = quarter * 32 + l2;
+                    const int i2 = (2 * pair + t) * beams_per_tile + r2 / G, g2 = r2 % G;
+                    if (i2 < n_q)
+                        *reinterpret_cast<float4*>(po + (row_base + (size_t)i2 * Hq + g2) * D + ch * 4) =
+                            *reinterpret_cast<const float4*>(stage + l2 * D + ((ch ^ (l2 & (CPR - 1))) * 4));
                 }
-            l_sum += psum;
-            // P buffer b was last read by the MMA of tile j-2
-            if (j >= 2) mbar_wait(bar_pvdone + 8 * b, (uint32_t)(((j - 2) >> 1) & 1));
-            __syncwarp();
-            tc_fence_after();
-            tmem_st32(lane_addr + C::COL_P + b * (BN / 2), pk[0]);
-            tmem_st32(lane_addr + C::COL_P + b * (BN / 2) + 32, pk[1]);
-            tmem_wait_st();
-            tc_fence_before();
-            mbar_arrive(bar_pfull + 8 * b);
-        }
-        // ---- epilogue: O row -> partials ----
-        mbar_wait(bar_pvdone + 8 * ((n_tiles - 1) & 1), (uint32_t)(((n_tiles - 1) >> 1) & 1));
-        __syncwarp();
-        tc_fence_after();
-        const int i = mt * beams_per_tile + r / G, g = r % G;
-        const bool live = i < n_q;
-        const size_t row = split * split_stride + ((size_t)u * n_q + (live ? i : 0)) * Hq + kv * G + g;
-        float4* o4 = reinterpret_cast<float4*>(po + row * D);
-#pragma unroll
-        for (int c = 0; c < D / 32; ++c) {
-            uint32_t o[32];
-            tmem_ld32(lane_addr + C::COL_O + c * 32, o);
-            tmem_wait_ld();
-            if (live) {
-#pragma unroll
-                for (int x = 0; x < 32; x += 4)
-                    o4[c * 8 + (x >> 2)] = make_float4(__uint_as_float(o[x]), __uint_as_float(o[x + 1]),
-                                                       __uint_as_float(o[x + 2]), __uint_as_float(o[x + 3]));
+                tc_fence_before();
             }
         }
-        if (live) { pm[row] = m_ref * kLn2; pl[row] = l_sum; }
-        tc_fence_before();
     }
     __syncthreads();
     if (warp == 1) {
@@ -452,7 +502,7 @@ int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const 
         attr_done = true;
     }
     const int M = n_q * p.G;
-    dim3 grid((M + BM - 1) / BM, p.Hkv * n_splits, p.B);
+    dim3 grid((M + 2 * BM - 1) / (2 * BM), p.Hkv * n_splits, p.B);  // one CTA per pair of Q tiles
     prefix_tc_kernel<D><<<grid, kThreadsTC, TcCfg<D>::SMEM_BYTES, st>>>(tq, tk, tv, cu, pm, pl, po, p.B, n_q, p.Hq,
                                                                        p.Hkv, p.G, n_splits, p.scale * kLog2e);
     STARK_LAUNCH_CHECK();
@@ -464,8 +514,8 @@ int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const 
 bool prefix_tc_supported(const Dims& p, int dtype, int n_q) {
     if (dtype != STARK_BF16) return false;
     if (p.D != 64 && p.D != 128) return false;
-    if (p.G > BM || (BM % p.G) != 0) return false;
-    return (long long)n_q * p.G >= 64;
+    (void)n_q;  // any number of queries: step 0 (M = G rows) streams the prefix through the same kernel
+    return p.G <= BM && (BM % p.G) == 0;
 }
 
 int launch_prefix_tc(const Dims& p, const void* q, int n_q, const void* k, const void* v, const int32_t* cu,

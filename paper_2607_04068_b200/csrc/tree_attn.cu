@@ -220,7 +220,9 @@ template <typename T, int D, int ML>
 int launch_m(const Dims& p, const void* q, int n_q, int level, const void* ks, const void* vs,
              const int32_t* anc_l, const float* pm, const float* pl, const float* po, int n_splits,
              void* out, cudaStream_t st) {
-    const int hpw = n_splits > 1 ? 1 : p.G;
+    // few queries with many prefix splits (decode step 0): one head per warp, for parallelism over the
+    // split partials; otherwise the whole GQA group per warp (the chain rows are fetched once per group)
+    const int hpw = (n_splits > 1 && (long long)p.B * n_q * p.Hkv < 2048) ? 1 : p.G;
     const long long warps = (long long)p.B * n_q * (p.Hq / hpw);
     const unsigned nb = (unsigned)((warps + kWarpsPerCta - 1) / kWarpsPerCta);
     const size_t smem = kWarpsPerCta * warp_region_bytes(hpw, D, (int)sizeof(T), level);
