@@ -69,6 +69,15 @@ def work_tree(cfg, n_q, level, n_splits):
     return rows * cfg.D * eb * 2 + n_splits * rows * (cfg.D + 2) * 4 + cfg.B * n_q * cfg.Hkv * 2 * level * cfg.D * eb
 
 
+def work_decode(cfg, lens, n_q, level):
+    """fused A1+A2: prefix K/V once, q in, chain rows, out -- no partials."""
+    eb, tot = cfg.elem_bytes, int(np.sum(lens))
+    flops = 4.0 * n_q * cfg.G * tot * cfg.D * cfg.Hkv
+    byts = 2.0 * cfg.D * eb * cfg.Hkv * tot + 2.0 * cfg.B * n_q * cfg.Hq * cfg.D * eb \
+        + cfg.B * n_q * cfg.Hkv * 2 * level * cfg.D * eb
+    return flops, byts
+
+
 def work_topk(cfg, W_in, W_out):
     return cfg.B * (W_in * cfg.C * 4 + W_in * 4 + W_out * 12)
 
@@ -327,12 +336,18 @@ def run_stark(args, cfg):
     kern = {}
     it = 40 * R
     for t in range(cfg.d):
-        ns = passes[0].layer.n_splits(nq[t])
-        fl, by = work_prefix(cfg, lens, nq[t], ns)
-        us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.prefix(p.q[t])) for p in passes], it, use_graph)
-        kern[f"prefix_attn.t{t}"] = {"us": us, "bytes": by, "flops": fl, "n_splits": ns}
-        us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.tree(t, p.q[t], p.out[t])) for p in passes], it, use_graph)
-        kern[f"tree_attn_step.t{t}"] = {"us": us, "bytes": work_tree(cfg, nq[t], t, ns)}
+        if passes[0].fused:
+            fl, by = work_decode(cfg, lens, nq[t], t)
+            us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.attend(t, p.q[t], out=p.out[t], fused=True))
+                                         for p in passes], it, use_graph)
+            kern[f"decode_attn.t{t}"] = {"us": us, "bytes": by, "flops": fl}
+        else:
+            ns = passes[0].layer.n_splits(nq[t])
+            fl, by = work_prefix(cfg, lens, nq[t], ns)
+            us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.prefix(p.q[t])) for p in passes], it, use_graph)
+            kern[f"prefix_attn.t{t}"] = {"us": us, "bytes": by, "flops": fl, "n_splits": ns}
+            us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.tree(t, p.q[t], p.out[t])) for p in passes], it, use_graph)
+            kern[f"tree_attn_step.t{t}"] = {"us": us, "bytes": work_tree(cfg, nq[t], t, ns)}
         w_in = nq[t]
         us = time_graph_loop(torch, [(lambda p=p, t=t: beam_topk(p.logp[t], p.sel[t - 1][0] if t else None, widths[t],
                                                                   out=p.sel[t])) for p in passes], it, use_graph)

@@ -172,6 +172,30 @@ int stark_tree_attn_step(const stark_shape_t* shape, const void* q, int n_q, int
                          int n_splits, void* out, void* stream);
 
 /* ---------------------------------------------------------------------------
+ * A1 + A2 fused: decode attention in ONE launch
+ *
+ * Same result as stark_prefix_attn followed by stark_tree_attn_step
+ * (every query attends to its user's whole prefix
+ * plus its own ancestor chain), but the split-softmax partials never leave the
+ * chip: the CTAs that share one (query tile pair, KV head, user) form a
+ * thread-block cluster over the prefix splits, exchange their partial rows
+ * through distributed shared memory, and the owner of each 32-row block merges
+ * them, adds the suffix chain and writes the normalised output.  Saves the
+ * fp32 partial round trip through HBM (2 * n_splits * B*n_q*Hq*(D+2)*4 bytes),
+ * the second read of q and one launch per step.
+ *
+ * Arguments as in the two separate calls; the split count (cluster size 1, 2,
+ * 4 or 8) is chosen from shapes only.  bf16 only: returns
+ * STARK_ERR_UNSUPPORTED for fp32 shapes (compose the two calls instead).
+ * Errors: INVALID_ARG (null pointers, level outside [0,d], n_q < 1, n_q > Wmax
+ * when level >= 1, total_tokens < 0, max_prefix_len < 1), UNSUPPORTED, CUDA.
+ */
+int stark_decode_attn(const stark_shape_t* shape, const void* q, int n_q, int level,
+                      const void* k_prefix, const void* v_prefix, const int32_t* cu_seqlens,
+                      int total_tokens, int max_prefix_len, const void* k_suffix,
+                      const void* v_suffix, const int32_t* anc, void* out, void* stream);
+
+/* ---------------------------------------------------------------------------
  * A3. Per-level beam selection
  *
  * Beam score = sum of per-level log-probabilities (Eq. 1);

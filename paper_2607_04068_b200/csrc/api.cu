@@ -84,6 +84,24 @@ int plan_splits(const Dims& p, int dtype, int n_q, int max_len) {
     return best;
 }
 
+// Cluster size (= prefix splits) of the fused decode-attention kernel: 1, 2, 4 or 8.  Same cost model;
+// the exchange through distributed shared memory costs about half a tile; resident CTAs: one per SM, whole
+// clusters only (B200 co-schedules 15 clusters of 8).
+int plan_cluster_splits(const Dims& p, int n_q, int max_len) {
+    const int sms = num_sms() > 0 ? num_sms() : 148;
+    const int tiles = ceil_div(max_len, 128);
+    const long long base = (long long)p.B * p.Hkv * ceil_div((long long)n_q * p.G, 256);
+    int best = 1;
+    double best_cost = 1e300;
+    for (int n = 1; n <= 8 && n <= tiles; n *= 2) {
+        const int resident = n == 8 ? (sms / 8 - 3) * 8 : sms / n * n;
+        const double waves = (double)ceil_div(base * n, resident > 0 ? resident : n);
+        const double cost = waves * (ceil_div(tiles, n) + 2.0 + (n > 1 ? 0.5 : 0.0));
+        if (cost < best_cost * 0.97) { best_cost = cost; best = n; }
+    }
+    return best;
+}
+
 }  // namespace
 }  // namespace stark
 
@@ -170,6 +188,25 @@ int stark_tree_attn_step(const stark_shape_t* shape, const void* q, int n_q, int
     if (rc != STARK_OK) return rc;
     return launch_tree_attn(make_dims(shape), shape->dtype, q, n_q, level, k_suffix, v_suffix, anc, part_m,
                             part_l, part_o, n_splits, out, (cudaStream_t)stream);
+}
+
+int stark_decode_attn(const stark_shape_t* shape, const void* q, int n_q, int level, const void* k_prefix,
+                      const void* v_prefix, const int32_t* cu_seqlens, int total_tokens, int max_prefix_len,
+                      const void* k_suffix, const void* v_suffix, const int32_t* anc, void* out, void* stream) {
+    int rc = check_shape(shape);
+    if (rc != STARK_OK) return rc;
+    if (!q || !cu_seqlens || !out) return STARK_ERR_INVALID_ARG;
+    if (n_q < 1 || total_tokens < 0 || max_prefix_len < 1 || level < 0 || level > shape->d) return STARK_ERR_INVALID_ARG;
+    if (total_tokens > 0 && (!k_prefix || !v_prefix)) return STARK_ERR_INVALID_ARG;
+    if (level >= 1 && (!k_suffix || !v_suffix || !anc || n_q > shape->Wmax)) return STARK_ERR_INVALID_ARG;
+    const Dims p = make_dims(shape);
+    if (!prefix_tc_supported(p, shape->dtype, n_q) || total_tokens < 1) return STARK_ERR_UNSUPPORTED;
+    rc = check_device();
+    if (rc != STARK_OK) return rc;
+    const int32_t* anc_l = anc ? anc + (size_t)(level & 1) * p.B * p.Wmax * p.d : nullptr;
+    return launch_decode_fused(p, q, n_q, level, k_prefix, v_prefix, cu_seqlens, total_tokens,
+                               plan_cluster_splits(p, n_q, max_prefix_len), k_suffix, v_suffix, anc_l, out,
+                               (cudaStream_t)stream);
 }
 
 int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_in, int C, int W_out,

@@ -172,6 +172,38 @@ __host__ __device__ constexpr uint32_t instr_desc(int M, int N, int b_mn_major) 
 }
 
 
+// ---- fused decode attention (A1 + A2 in one launch) ---------------------------------
+// Arguments of the suffix / merge / normalise tail that replaces the partial epilogue.
+struct FusedArgs {
+    const __nv_bfloat16* q;    // [B, n_q, Hq, D]
+    const __nv_bfloat16* ks;   // suffix K [d, B, Wmax, Hkv, D]
+    const __nv_bfloat16* vs;
+    const int32_t* anc;        // this level's half of the ancestor index, [B, Wmax, d]
+    __nv_bfloat16* out;        // [B, n_q, Hq, D]
+    int level, Wmax, d;
+    float scale;               // softmax scale (natural units)
+};
+
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t cluster_rank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t map_to_rank(uint32_t smem_addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_cluster_f4(uint32_t addr, float a, float b, float c, float d) {
+    asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+__device__ __forceinline__ void st_cluster_f2(uint32_t addr, float a, float b) {
+    asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
+}
+
 template <int D> struct TcCfg {
     static constexpr int BOXES = D / 64;                 // 64-element (128-byte) column boxes per row
     static constexpr int TILE_BYTES = BOXES * BM * 128;  // one 128-row tile of Q, K or V
@@ -182,17 +214,164 @@ template <int D> struct TcCfg {
     static constexpr int COL_O = 256;                    // O_t at COL_O + t * 128
 };
 
+// Tail of the fused kernel, run by the warp that owns one 32-row block (lane = row): merge the block's
+// prefix partials of all splits (own rows in TMEM, the others' delivered into the K/V ring), add the suffix
+// chain of each row (Eq. 14: ancestors and itself), normalise, write bf16 rows coalesced.
+// Runs once per CTA, so it is written for SMALL CODE (rolled loops, per-lane scratch in shared memory): a
+// fully unrolled version was instruction-fetch bound (~100 KB of straight-line code: 16 us).
 template <int D>
+__device__ __noinline__ void fused_finish(const FusedArgs& fa, unsigned char* smem_raw, uint32_t ring_off, int ob, int me,
+                                          int ns, int lane, uint32_t aO, bool has, float m_own, float l_own,
+                                          float scale_log2, int u, int n_q, int Hq, int Hkv, int G, int kv,
+                                          int beam_base, int quarter, int B) {
+    constexpr uint32_t SLOT = 32 * D * 4;
+    constexpr int CPR = D / 4;                          // 16-byte chunks per fp32 row
+    constexpr int CPO = D / 8;                          // 16-byte chunks per bf16 row
+    unsigned char* ring = smem_raw + ring_off;
+    // this block's own slot is never written remotely: bf16 output staging [32][D] + per-lane scratch
+    unsigned char* stage = ring + (size_t)(ob * ns + me) * SLOT;
+    float* wgt = reinterpret_cast<float*>(stage + 32 * D * 2);          // [16][32]: split weights 0..7, chain 8..15
+    uint32_t* voff = reinterpret_cast<uint32_t*>(wgt + 16 * 32);          // [8][32]: element offset of the V row
+    const int r = quarter * 32 + lane;
+    const int i = beam_base + r / G, g = r % G;
+    const bool live = i < n_q;
+    const int level = fa.level;
+    const size_t level_stride = (size_t)B * fa.Wmax * Hkv * D;
+    tc_fence_after();
+
+    // ---- chain scores (log2 units) -> wgt[8 + t], row offsets -> voff[t] ----------------------------------
+    float m_all = has ? m_own : -INFINITY;
+    if (level > 0) {
+        uint4 qv[D / 8];
+        const uint4* qp = reinterpret_cast<const uint4*>(fa.q + (((size_t)u * n_q + (live ? i : 0)) * Hq + kv * G + g) * D);
+#pragma unroll
+        for (int c = 0; c < D / 8; ++c) qv[c] = __ldg(qp + c);
+#pragma unroll 1
+        for (int t = 0; t < level; ++t) {
+            int a = __ldg(fa.anc + ((size_t)u * fa.Wmax + (live ? i : 0)) * fa.d + t);
+            a = min(max(a, 0), fa.Wmax - 1);            // memory safety on garbage input
+            const size_t off = (size_t)t * level_stride + (((size_t)u * fa.Wmax + a) * Hkv + kv) * D;
+            const uint4* kp = reinterpret_cast<const uint4*>(fa.ks + off);
+            float dot = 0.f;
+#pragma unroll
+            for (int c = 0; c < D / 8; ++c) {
+                const uint4 kk = __ldg(kp + c);
+                const uint32_t qa[4] = {qv[c].x, qv[c].y, qv[c].z, qv[c].w}, ka[4] = {kk.x, kk.y, kk.z, kk.w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    dot = fmaf(__uint_as_float(qa[e] << 16), __uint_as_float(ka[e] << 16), dot);
+                    dot = fmaf(__uint_as_float(qa[e] & 0xffff0000u), __uint_as_float(ka[e] & 0xffff0000u), dot);
+                }
+            }
+            const float yt = dot * scale_log2;
+            wgt[(8 + t) * 32 + lane] = yt;
+            voff[t * 32 + lane] = (uint32_t)off;        // suffix buffers are far below 2^32 elements
+            m_all = fmaxf(m_all, yt);
+        }
+    }
+    // ---- log-sum-exp weights over {own split, delivered splits, chain} ------------------------------------
+#pragma unroll 1
+    for (int sidx = 0; sidx < ns; ++sidx)
+        if (sidx != me) m_all = fmaxf(m_all, *reinterpret_cast<const float*>(ring + 8 * SLOT + (size_t)(ob * ns + sidx) * 256 + lane * 8));
+    const bool any = m_all > -INFINITY;                 // false only for an empty prefix at level 0
+    const float w_own = (has && any && m_own > -INFINITY) ? fast_exp2(m_own - m_all) : 0.f;
+    float denom = w_own * l_own;
+#pragma unroll 1
+    for (int sidx = 0; sidx < ns; ++sidx) {
+        if (sidx == me) continue;
+        const float2 v = *reinterpret_cast<const float2*>(ring + 8 * SLOT + (size_t)(ob * ns + sidx) * 256 + lane * 8);
+        const float w = (any && v.x > -INFINITY) ? fast_exp2(v.x - m_all) : 0.f;
+        wgt[sidx * 32 + lane] = w;
+        denom = fmaf(w, v.y, denom);
+    }
+#pragma unroll 1
+    for (int t = 0; t < level; ++t) {
+        const float e = (any && live) ? fast_exp2(wgt[(8 + t) * 32 + lane] - m_all) : 0.f;
+        wgt[(8 + t) * 32 + lane] = e;
+        denom += e;
+    }
+    const float inv = denom > 0.f ? 1.0f / denom : 0.f;
+
+    // ---- output row, 32 columns at a time ---------------------------------------------------------------------
+#pragma unroll 1
+    for (int c = 0; c < D / 32; ++c) {
+        float acc[32];
+        {
+            uint32_t o[32];
+            tmem_ld32(aO + c * 32, o);
+            tmem_wait_ld();
+#pragma unroll
+            for (int x = 0; x < 32; ++x) acc[x] = has ? w_own * __uint_as_float(o[x]) : 0.f;
+        }
+#pragma unroll 1
+        for (int sidx = 0; sidx < ns; ++sidx) {
+            if (sidx == me) continue;
+            const float w = wgt[sidx * 32 + lane];
+            const float* src = reinterpret_cast<const float*>(ring + (size_t)(ob * ns + sidx) * SLOT) + lane * D;
+#pragma unroll
+            for (int x = 0; x < 32; x += 4) {
+                const float4 v = *reinterpret_cast<const float4*>(src + (((c * 8 + (x >> 2)) ^ (lane & (CPR - 1))) * 4));
+                acc[x] = fmaf(w, v.x, acc[x]); acc[x + 1] = fmaf(w, v.y, acc[x + 1]);
+                acc[x + 2] = fmaf(w, v.z, acc[x + 2]); acc[x + 3] = fmaf(w, v.w, acc[x + 3]);
+            }
+        }
+#pragma unroll 1
+        for (int t = 0; t < level; ++t) {
+            const float e = wgt[(8 + t) * 32 + lane];
+            const uint4* vp = reinterpret_cast<const uint4*>(fa.vs + voff[t * 32 + lane]) + c * 4;
+#pragma unroll
+            for (int k4 = 0; k4 < 4; ++k4) {
+                const uint4 vv = __ldg(vp + k4);
+                const uint32_t va[4] = {vv.x, vv.y, vv.z, vv.w};
+#pragma unroll
+                for (int e2 = 0; e2 < 4; ++e2) {
+                    acc[k4 * 8 + 2 * e2] = fmaf(e, __uint_as_float(va[e2] << 16), acc[k4 * 8 + 2 * e2]);
+                    acc[k4 * 8 + 2 * e2 + 1] = fmaf(e, __uint_as_float(va[e2] & 0xffff0000u), acc[k4 * 8 + 2 * e2 + 1]);
+                }
+            }
+        }
+#pragma unroll
+        for (int k4 = 0; k4 < 4; ++k4) {                // 4 chunks of 8 bf16
+            uint32_t pk[4];
+#pragma unroll
+            for (int e2 = 0; e2 < 4; ++e2) {
+                const __nv_bfloat162 h = __floats2bfloat162_rn(acc[k4 * 8 + 2 * e2] * inv, acc[k4 * 8 + 2 * e2 + 1] * inv);
+                pk[e2] = *reinterpret_cast<const uint32_t*>(&h);
+            }
+            const int ch = (c * 4 + k4) ^ (lane & (CPO - 1));
+            *reinterpret_cast<uint4*>(stage + (size_t)lane * D * 2 + ch * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        }
+    }
+    __syncwarp();
+    const size_t row_base = (size_t)u * n_q * Hq + kv * G;
+#pragma unroll 1
+    for (int idx = lane; idx < 32 * CPO; idx += 32) {
+        const int l2 = idx / CPO, ch = idx % CPO;
+        const int r2 = quarter * 32 + l2;
+        const int i2 = beam_base + r2 / G, g2 = r2 % G;
+        if (i2 < n_q)
+            *reinterpret_cast<uint4*>(fa.out + (row_base + (size_t)i2 * Hq + g2) * D + ch * 8) =
+                *reinterpret_cast<const uint4*>(stage + (size_t)l2 * D * 2 + ((ch ^ (l2 & (CPO - 1))) * 16));
+    }
+}
+
+// FUSED = false: emit the split-softmax partials (stark_prefix_attn).
+// FUSED = true : the n_splits CTAs of one (Q-tile pair, KV head, user) form a thread-block cluster; they
+//                exchange their partial rows through distributed shared memory, and the owner of each
+//                32-row block merges them, adds the suffix chain and writes the normalised bf16 output
+//                (stark_decode_attn): no partial ever goes to HBM.
+template <int D, bool FUSED>
 __global__ void __launch_bounds__(kThreadsTC, 1)
 prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                  const __grid_constant__ CUtensorMap tm_v, const int32_t* __restrict__ cu,
                  float* __restrict__ pm, float* __restrict__ pl, float* __restrict__ po, int B, int n_q,
-                 int Hq, int Hkv, int G, int n_splits, float scale_log2) {
+                 int Hq, int Hkv, int G, int n_splits, float scale_log2, const FusedArgs fa) {
     using C = TcCfg<D>;
     constexpr int NS = C::NS;
     const int pair = blockIdx.x;                         // Q tiles 2*pair and 2*pair + 1
-    const int kv = blockIdx.y % Hkv;
-    const int split = blockIdx.y / Hkv;
+    // FUSED: the splits of one KV head are adjacent in y (cluster dims (1, n_splits, 1))
+    const int kv = FUSED ? blockIdx.y / n_splits : blockIdx.y % Hkv;
+    const int split = FUSED ? blockIdx.y % n_splits : blockIdx.y / Hkv;
     const int u = blockIdx.z;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -208,7 +387,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     const bool two = M > (2 * pair + 1) * BM;            // does the second Q tile hold any live row?
     const size_t split_stride = (size_t)B * n_q * Hq;
 
-    if (n_tiles == 0) {  // empty split: (m, l, o) = (-inf, 0, 0), reading R18
+    if (!FUSED && n_tiles == 0) {  // empty split: (m, l, o) = (-inf, 0, 0), reading R18
         if (warp >= 2) {
             const int t = (warp - 2) >> 2;
             const int r = (threadIdx.x - 64) & 127;
@@ -262,12 +441,14 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
         fence_barrier_init();
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         const int beam0 = u * n_q + 2 * pair * beams_per_tile;
-        mbar_expect_tx(bar_q, (two ? 2 : 1) * C::TILE_BYTES);
-        for (int t = 0; t < (two ? 2 : 1); ++t)
+        if (n_tiles > 0) {                               // (a fused CTA with an empty split loads nothing)
+            mbar_expect_tx(bar_q, (two ? 2 : 1) * C::TILE_BYTES);
+            for (int t = 0; t < (two ? 2 : 1); ++t)
 #pragma unroll
-            for (int bx = 0; bx < C::BOXES; ++bx)
-                tma_load_3d(sQ + t * C::TILE_BYTES + bx * (BM * 128), &tm_q, bar_q, bx * 64, kv * G,
-                            beam0 + t * beams_per_tile);
+                for (int bx = 0; bx < C::BOXES; ++bx)
+                    tma_load_3d(sQ + t * C::TILE_BYTES + bx * (BM * 128), &tm_q, bar_q, bx * 64, kv * G,
+                                beam0 + t * beams_per_tile);
+        }
         for (; n_issued < min(NS, 2 * n_tiles); ++n_issued) issue_kv(n_issued);  // the ring starts empty
     }
     if (warp == 1) tmem_alloc(tmem_slot, C::TMEM_COLS);
@@ -275,6 +456,17 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot_ptr;
+
+    // identity of a softmax warp (warps 2..9; harmless values for warps 0 and 1)
+    const int t = (warp - 2) >> 2;                      // Q tile (= warpgroup) of this warp
+    const int quarter = warp & 3;                       // TMEM lane quarter this warp may access
+    const int r = quarter * 32 + lane;                  // query row inside the Q tile
+    const int i = (2 * pair + t) * beams_per_tile + r / G, g = r % G;
+    const bool live = warp >= 2 && i < n_q;
+    const bool warp_live = __any_sync(0xffffffffu, live);
+    const uint32_t lane_addr = tmem + ((uint32_t)(quarter * 32) << 16);
+    const uint32_t aO = lane_addr + C::COL_O + t * 128;
+    float m_ref = -INFINITY, l_sum = 0.f;               // m_ref in log2 units of the scaled score
 
     if (warp == 0) {
         // ===================== TMA producer (rest of the stream) =====================
@@ -286,7 +478,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
         }
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
-        if (lane == 0) {
+        if (lane == 0 && n_tiles > 0) {
             constexpr uint32_t idesc_s = instr_desc(BM, BN, 0);
             constexpr uint32_t idesc_o = instr_desc(BM, D, 1);
             // S_t = Q_t K_j^T; K_j sits in ring slot s
@@ -332,16 +524,8 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
         }
     } else {
         // ===================== softmax / correction / epilogue =====================
-        const int t = (warp - 2) >> 2;                  // Q tile (= warpgroup) of this warp
-        const int quarter = warp & 3;                   // TMEM lane quarter this warp may access
-        const int r = quarter * 32 + lane;              // query row inside the Q tile
-        const int i = (2 * pair + t) * beams_per_tile + r / G, g = r % G;
-        const bool live = i < n_q;
-        const bool warp_live = __any_sync(0xffffffffu, live);
         if (t == 0 || two) {
-            const uint32_t lane_addr = tmem + ((uint32_t)(quarter * 32) << 16);
-            const uint32_t aS = lane_addr + C::COL_S + t * BN, aO = lane_addr + C::COL_O + t * 128;
-            float m_ref = -INFINITY, l_sum = 0.f;       // m_ref in log2 units of the scaled score
+            const uint32_t aS = lane_addr + C::COL_S + t * BN;
             for (int j = 0; j < n_tiles; ++j) {
                 mbar_wait(bar_sfull + 8 * t, (uint32_t)(j & 1));
                 __syncwarp();
@@ -415,9 +599,9 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 mbar_arrive(bar_pfull + 8 * t);
             }
             // ---- epilogue: O row -> partials ----
-            mbar_wait(bar_done, 0);
+            if (n_tiles > 0) mbar_wait(bar_done, 0);
             __syncwarp();
-            if (warp_live) {
+            if (!FUSED && warp_live) {
                 tc_fence_after();
                 // Each thread owns one O row (512 B), so direct stores would scatter 16-byte pieces over 32
                 // rows per instruction (measured: 5.5 us for 17 MB).  Stage the warp's 32 rows in the (now
@@ -451,6 +635,43 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 tc_fence_before();
             }
         }
+    }
+    if constexpr (FUSED) {
+        const bool mine = warp >= 2 && (t == 0 || two) && warp_live;  // this warp's 32-row block has live rows
+        const int blk = t * 4 + quarter;                               // 32-row block of the 256-row pair
+        const int owner = blk % n_splits, ob = blk / n_splits;         // cluster rank that finishes it
+        const uint32_t me = n_splits > 1 ? cluster_rank() : 0u;
+        constexpr uint32_t SLOT = 32 * D * 4;                          // one block of fp32 O rows
+        const uint32_t ml_base = sKV + 8 * SLOT;                       // (m, l) pairs: [slot][32][2]
+        // B1: every CTA of the cluster is done with its K/V ring, which now becomes the exchange buffer
+        if (n_splits > 1) cluster_sync_all();
+        if (mine && owner != (int)me) {
+            tc_fence_after();
+            const uint32_t slot = (uint32_t)(ob * n_splits) + me;
+            const uint32_t dst = map_to_rank(sKV + slot * SLOT + (uint32_t)lane * D * 4, (uint32_t)owner);
+            constexpr int CPR = D / 4;
+#pragma unroll
+            for (int c = 0; c < D / 32; ++c) {
+                uint32_t o[32];
+                tmem_ld32(aO + c * 32, o);
+                tmem_wait_ld();
+#pragma unroll
+                for (int x = 0; x < 32; x += 4) {
+                    const int ch = (c * 8 + (x >> 2)) ^ (lane & (CPR - 1));
+                    if (n_tiles > 0)
+                        st_cluster_f4(dst + ch * 16, __uint_as_float(o[x]), __uint_as_float(o[x + 1]),
+                                      __uint_as_float(o[x + 2]), __uint_as_float(o[x + 3]));
+                    else
+                        st_cluster_f4(dst + ch * 16, 0.f, 0.f, 0.f, 0.f);  // empty split: (-inf, 0, 0)
+                }
+            }
+            st_cluster_f2(map_to_rank(ml_base + slot * 256 + (uint32_t)lane * 8, (uint32_t)owner), m_ref, l_sum);
+        }
+        if (n_splits > 1) cluster_sync_all();                          // B2: all partial rows delivered
+        if (mine && owner == (int)me)
+            fused_finish<D>(fa, smem_raw, sKV - smem_u32(smem_raw), ob, (int)me, n_splits, lane, aO, n_tiles > 0, m_ref,
+                            l_sum, scale_log2, u, n_q, Hq, Hkv, G, kv, (2 * pair + t) * beams_per_tile, quarter, B);
+        tc_fence_before();
     }
     __syncthreads();
     if (warp == 1) {
@@ -497,15 +718,41 @@ int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const 
              const int32_t* cu, int n_splits, float* pm, float* pl, float* po, cudaStream_t st) {
     static bool attr_done = false;
     if (!attr_done) {
-        STARK_CUDA_TRY(cudaFuncSetAttribute(prefix_tc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        STARK_CUDA_TRY(cudaFuncSetAttribute(prefix_tc_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             TcCfg<D>::SMEM_BYTES));
         attr_done = true;
     }
     const int M = n_q * p.G;
     dim3 grid((M + 2 * BM - 1) / (2 * BM), p.Hkv * n_splits, p.B);  // one CTA per pair of Q tiles
-    prefix_tc_kernel<D><<<grid, kThreadsTC, TcCfg<D>::SMEM_BYTES, st>>>(tq, tk, tv, cu, pm, pl, po, p.B, n_q, p.Hq,
-                                                                       p.Hkv, p.G, n_splits, p.scale * kLog2e);
+    prefix_tc_kernel<D, false><<<grid, kThreadsTC, TcCfg<D>::SMEM_BYTES, st>>>(
+        tq, tk, tv, cu, pm, pl, po, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits, p.scale * kLog2e, FusedArgs{});
     STARK_LAUNCH_CHECK();
+    return STARK_OK;
+}
+
+// fused launch: the n_splits CTAs of one (pair, KV head, user) are a cluster along y
+template <int D>
+int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, int n_q,
+                   const int32_t* cu, int n_splits, const FusedArgs& fa, cudaStream_t st) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        STARK_CUDA_TRY(cudaFuncSetAttribute(prefix_tc_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            TcCfg<D>::SMEM_BYTES));
+        attr_done = true;
+    }
+    const int M = n_q * p.G;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((M + 2 * BM - 1) / (2 * BM), p.Hkv * n_splits, p.B);
+    cfg.blockDim = dim3(kThreadsTC);
+    cfg.dynamicSmemBytes = TcCfg<D>::SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = n_splits; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    STARK_CUDA_TRY(cudaLaunchKernelEx(&cfg, prefix_tc_kernel<D, true>, tq, tk, tv, cu, (float*)nullptr,
+                                      (float*)nullptr, (float*)nullptr, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits,
+                                      p.scale * kLog2e, fa));
     return STARK_OK;
 }
 
@@ -530,6 +777,24 @@ int launch_prefix_tc(const Dims& p, const void* q, int n_q, const void* k, const
     }
     if (p.D == 128) return launch_d<128>(p, tq, tk, tv, n_q, cu, n_splits, pm, pl, po, st);
     return launch_d<64>(p, tq, tk, tv, n_q, cu, n_splits, pm, pl, po, st);
+}
+
+// A1 + A2 in one launch (bf16): n_splits in {1, 2, 4, 8} = cluster size along the prefix.
+int launch_decode_fused(const Dims& p, const void* q, int n_q, int level, const void* k, const void* v,
+                        const int32_t* cu, int total_tokens, int n_splits, const void* ks, const void* vs,
+                        const int32_t* anc_level, void* out, cudaStream_t st) {
+    CUtensorMap tq, tk, tv;
+    if (!make_map(&tq, q, p.D, p.Hq, (long long)p.B * n_q, p.G, BM / p.G) ||
+        !make_map(&tk, k, p.D, p.Hkv, total_tokens, 1, BN) || !make_map(&tv, v, p.D, p.Hkv, total_tokens, 1, BN)) {
+        last_cuda_error_ref() = (int)cudaErrorInvalidValue;
+        return STARK_ERR_CUDA;
+    }
+    FusedArgs fa;
+    fa.q = (const __nv_bfloat16*)q; fa.ks = (const __nv_bfloat16*)ks; fa.vs = (const __nv_bfloat16*)vs;
+    fa.anc = anc_level; fa.out = (__nv_bfloat16*)out;
+    fa.level = level; fa.Wmax = p.Wmax; fa.d = p.d; fa.scale = p.scale;
+    if (p.D == 128) return launch_fused_d<128>(p, tq, tk, tv, n_q, cu, n_splits, fa, st);
+    return launch_fused_d<64>(p, tq, tk, tv, n_q, cu, n_splits, fa, st);
 }
 
 }  // namespace stark

@@ -59,12 +59,21 @@ class StarkLayer:
                                 self.anc if anc is None else anc, pm, pl, po, ns, out)
 
     def attend(self, level: int, q: torch.Tensor, out: Optional[torch.Tensor] = None,
-               anc: Optional[torch.Tensor] = None) -> torch.Tensor:
-        """Attention of the level-`level` queries q[B,n_q,Hq,D] over prefix + ancestor chain."""
+               anc: Optional[torch.Tensor] = None, fused: Optional[bool] = None) -> torch.Tensor:
+        """Attention of the level-`level` queries q[B,n_q,Hq,D] over prefix + ancestor chain.
+        bf16: one fused launch (stark_decode_attn); fp32 (or fused=False): stark_prefix_attn followed by
+        stark_tree_attn_step."""
         if out is None:
             out = torch.empty_like(q)
-        self.prefix(q)
-        self.tree(level, q, out, anc)
+        if fused is None:
+            fused = self.dtype == torch.bfloat16 and self.total_tokens > 0
+        if fused:
+            sb.stark_decode_attn(self.shape, q, int(q.shape[1]), level, self.k_prefix, self.v_prefix, self.cu,
+                                 self.total_tokens, self.max_len, self.k_suffix, self.v_suffix,
+                                 self.anc if anc is None else anc, out)
+        else:
+            self.prefix(q)
+            self.tree(level, q, out, anc)
         return out
 
     def n_splits(self, n_q: int) -> int:

@@ -1,5 +1,6 @@
 """One whole pass of the STARK hot path (all rows of SURVEY.md section 8(a)) for one batch:
-decode steps t = 0..d-1, each  append(t>=1) -> prefix_attn -> tree_attn_step -> beam_topk.
+decode steps t = 0..d-1, each  append(t>=1) -> decode attention -> beam_topk, where decode attention is
+the fused stark_decode_attn launch for bf16 and stark_prefix_attn -> stark_tree_attn_step for fp32.
 
 Inputs (prefix K/V, per-step q / k_new / v_new, per-level log-probs) are device tensors;
 `DecodePass.run()` only enqueues library calls on the current stream, so a pass is CUDA-graph
@@ -22,8 +23,9 @@ class DecodePass:
                  logp: List[torch.Tensor]):
         self.B, self.d, self.C, self.widths = B, d, C, list(widths)
         self.n_q = [1] + self.widths                      # queries per user at step t
+        self.fused = dtype == torch.bfloat16 and int(k_prefix.shape[0]) > 0
         self.layer = StarkLayer(B, Hq, Hkv, D, d, max(self.widths), dtype, k_prefix, v_prefix, cu_seqlens,
-                                max_prefix_len, n_q_per_step=self.n_q[:d])
+                                max_prefix_len, n_q_per_step=None if self.fused else self.n_q[:d])
         self.q, self.k_new, self.v_new, self.logp = q, k_new, v_new, logp
         dev = k_prefix.device
         self.out = [torch.empty_like(q[t]) for t in range(d)]
@@ -31,17 +33,17 @@ class DecodePass:
                      torch.empty((B, w), dtype=torch.int32, device=dev),
                      torch.empty((B, w), dtype=torch.int32, device=dev)) for w in self.widths]
 
-    #: library kernels launched by one run(): step 0 = 3, steps >= 1 = 4 each
+    #: library kernels launched by one run(): attention (1 fused or 2) + top-k per step, + append for t >= 1
     @property
     def launches(self) -> int:
-        return 3 + 4 * (self.d - 1)
+        return (2 if self.fused else 3) * self.d + (self.d - 1)
 
     def run(self) -> None:
         score = parent = None
         for t in range(self.d):
             if t >= 1:
                 self.layer.append(t, self.k_new[t], self.v_new[t], parent)
-            self.layer.attend(t, self.q[t], out=self.out[t])
+            self.layer.attend(t, self.q[t], out=self.out[t], fused=self.fused)
             score, parent, _ = beam_topk(self.logp[t], score, self.widths[t], out=self.sel[t])
 
     def result(self) -> Dict[str, List[torch.Tensor]]:

@@ -82,10 +82,12 @@ def run_teacher_forced(cfg, seed=0, final_step=True):
             kn = np.stack([tr[u].k_new[t] for u in range(cfg.B)]).astype(np.float32)
             vn = np.stack([tr[u].v_new[t] for u in range(cfg.B)]).astype(np.float32)
             layer.append(t, to_dev(kn, dt), to_dev(vn, dt), parent)
-        out = layer.attend(t, q).float().cpu().numpy().astype(np.float64)
         ref = np.stack([tr[u].attn_out[t] for u in range(cfg.B)])
-        err = np.abs(out - ref).max() / np.abs(ref).max()
-        report.append(("attn", t, bool(np.isfinite(out).all() and err <= tol), f"rel_err={err:.3e} tol={tol}"))
+        # both boundaries: A1 then A2 (partials through HBM), and the fused single launch (bf16 only)
+        for what, fused in (("attn", False),) + ((("attn_fused", True),) if cfg.dtype == "bf16" else ()):
+            out = layer.attend(t, q, fused=fused).float().cpu().numpy().astype(np.float64)
+            err = np.abs(out - ref).max() / np.abs(ref).max()
+            report.append((what, t, bool(np.isfinite(out).all() and err <= tol), f"rel_err={err:.3e} tol={tol}"))
         if t == cfg.d:
             break
         logp = np.stack([tr[u].logp[t] for u in range(cfg.B)])            # fp32, the oracle's O3 output
