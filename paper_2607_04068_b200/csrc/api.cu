@@ -68,35 +68,47 @@ int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 // prologue allocates TMEM and fills the TMA ring); ties go to the smaller
 // split count (less partial traffic).
 int plan_splits(const Dims& p, int dtype, int n_q, int max_len) {
-    const int sms = num_sms();
+    const int sms = num_sms() > 0 ? num_sms() : 148;
     const int tiles = ceil_div(max_len, 128);
     const bool tc = prefix_tc_supported(p, dtype, n_q);
     const long long M = (long long)n_q * p.G;
-    const long long base = (long long)p.B * p.Hkv * (tc ? ceil_div(M, 256) : ceil_div(M, 4));  // CTAs per split
-    const int per_sm = tc ? 1 : 4;  // resident CTAs per SM of each kernel
     int best = 1;
     double best_cost = 1e300;
     for (int n = 1; n <= 64 && n <= tiles; ++n) {
-        const double waves = (double)ceil_div(base * n, (long long)sms * per_sm);
-        const double cost = waves * (ceil_div(tiles, n) + (tc ? 2.0 : 1.0));
+        double cost;
+        if (tc) {
+            // tensor-core kernel: an iteration handles one KV tile for a Q-tile pair, or (parity mode, when the
+            // doubled CTA count still fits one wave) two KV tiles for one Q tile; ~2 iterations of prologue /
+            // epilogue; every extra split adds a partial set (fp32, written and re-read through HBM)
+            const bool parity = prefix_tc_parity(p, n_q, n);
+            const long long ctas = (long long)p.B * p.Hkv * n * ceil_div(M, parity ? 128 : 256);
+            const double iters = parity ? ceil_div(ceil_div(tiles, n), 2) + 0.5 : ceil_div(tiles, n);
+            cost = (double)ceil_div(ctas, sms) * (iters + 2.0) + 0.75 * (n - 1);
+        } else {
+            const long long ctas = (long long)p.B * p.Hkv * n * ceil_div(M, 4);
+            cost = (double)ceil_div(ctas, (long long)sms * 4) * (ceil_div(tiles, n) + 1.0);
+        }
         if (cost < best_cost * 0.97) { best_cost = cost; best = n; }
     }
     return best;
 }
 
-// Cluster size (= prefix splits) of the fused decode-attention kernel: 1, 2, 4 or 8.  Same cost model;
-// the exchange through distributed shared memory costs about half a tile; resident CTAs: one per SM, whole
-// clusters only (B200 co-schedules 15 clusters of 8).
+// Cluster size (= prefix splits) of the fused decode-attention kernel: 1, 2, 4 or 8.  Same cost model; the
+// exchange through distributed shared memory (~17 B/clk per SM) costs up to ~3.5 iterations when all 256
+// rows are live; resident CTAs: one per SM, whole clusters only (B200 co-schedules 15 clusters of 8).
 int plan_cluster_splits(const Dims& p, int n_q, int max_len) {
     const int sms = num_sms() > 0 ? num_sms() : 148;
     const int tiles = ceil_div(max_len, 128);
-    const long long base = (long long)p.B * p.Hkv * ceil_div((long long)n_q * p.G, 256);
+    const long long M = (long long)n_q * p.G;
     int best = 1;
     double best_cost = 1e300;
     for (int n = 1; n <= 8 && n <= tiles; n *= 2) {
+        const bool parity = prefix_tc_parity(p, n_q, n);
+        const long long ctas = (long long)p.B * p.Hkv * n * ceil_div(M, parity ? 128 : 256);
         const int resident = n == 8 ? (sms / 8 - 3) * 8 : sms / n * n;
-        const double waves = (double)ceil_div(base * n, resident > 0 ? resident : n);
-        const double cost = waves * (ceil_div(tiles, n) + 2.0 + (n > 1 ? 0.5 : 0.0));
+        const double iters = parity ? ceil_div(ceil_div(tiles, n), 2) + 0.5 : ceil_div(tiles, n);
+        const double live = (double)(M < 256 ? M : 256) / 256.0;
+        const double cost = (double)ceil_div(ctas, resident > 0 ? resident : n) * (iters + 2.0) + (n > 1 ? 3.5 * live : 0.0);
         if (cost < best_cost * 0.97) { best_cost = cost; best = n; }
     }
     return best;

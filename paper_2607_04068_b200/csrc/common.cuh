@@ -95,6 +95,7 @@ int launch_prefix_tc(const Dims& p, const void* q, int n_q, const void* k, const
                      const int32_t* cu, int total_tokens, int n_splits, float* pm, float* pl,
                      float* po, cudaStream_t st);
 bool prefix_tc_supported(const Dims& p, int dtype, int n_q);
+bool prefix_tc_parity(const Dims& p, int n_q, int n_splits);
 int launch_decode_fused(const Dims& p, const void* q, int n_q, int level, const void* k, const void* v,
                         const int32_t* cu, int total_tokens, int n_splits, const void* ks, const void* vs,
                         const int32_t* anc_level, void* out, cudaStream_t st);

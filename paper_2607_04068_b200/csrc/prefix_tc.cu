@@ -214,6 +214,39 @@ template <int D> struct TcCfg {
     static constexpr int COL_O = 256;                    // O_t at COL_O + t * 128
 };
 
+// Suffix-chain scores of one query row (Eq. 14: ancestors and itself), in log2 units of the
+// scaled score, and the element offsets of the chain's rows in the suffix buffers.  Independent of the prefix,
+// so the fused kernel runs it while the first K/V tiles are still in flight.
+template <int D>
+__device__ __noinline__ void chain_scores(const FusedArgs& fa, float scale_log2, int u, int i, int h, int kv, int n_q,
+                                          int Hq, int Hkv, int B, float* y, uint32_t* off_out) {
+    const size_t level_stride = (size_t)B * fa.Wmax * Hkv * D;
+    uint4 qv[D / 8];
+    const uint4* qp = reinterpret_cast<const uint4*>(fa.q + (((size_t)u * n_q + i) * Hq + h) * D);
+#pragma unroll
+    for (int c = 0; c < D / 8; ++c) qv[c] = __ldg(qp + c);
+#pragma unroll 1
+    for (int t = 0; t < fa.level; ++t) {
+        int a = __ldg(fa.anc + ((size_t)u * fa.Wmax + i) * fa.d + t);
+        a = min(max(a, 0), fa.Wmax - 1);                // memory safety on garbage input
+        const size_t off = (size_t)t * level_stride + (((size_t)u * fa.Wmax + a) * Hkv + kv) * D;
+        const uint4* kp = reinterpret_cast<const uint4*>(fa.ks + off);
+        float dot = 0.f;
+#pragma unroll
+        for (int c = 0; c < D / 8; ++c) {
+            const uint4 kk = __ldg(kp + c);
+            const uint32_t qa[4] = {qv[c].x, qv[c].y, qv[c].z, qv[c].w}, ka[4] = {kk.x, kk.y, kk.z, kk.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                dot = fmaf(__uint_as_float(qa[e] << 16), __uint_as_float(ka[e] << 16), dot);
+                dot = fmaf(__uint_as_float(qa[e] & 0xffff0000u), __uint_as_float(ka[e] & 0xffff0000u), dot);
+            }
+        }
+        y[t] = dot * scale_log2;
+        off_out[t] = (uint32_t)off;                     // suffix buffers are far below 2^32 elements
+    }
+}
+
 // Tail of the fused kernel, run by the warp that owns one 32-row block (lane = row): merge the block's
 // prefix partials of all splits (own rows in TMEM, the others' delivered into the K/V ring), add the suffix
 // chain of each row (Eq. 14: ancestors and itself), normalise, write bf16 rows coalesced.
@@ -222,53 +255,23 @@ template <int D> struct TcCfg {
 template <int D>
 __device__ __noinline__ void fused_finish(const FusedArgs& fa, unsigned char* smem_raw, uint32_t ring_off, int ob, int me,
                                           int ns, int lane, uint32_t aO, bool has, float m_own, float l_own,
-                                          float scale_log2, int u, int n_q, int Hq, int Hkv, int G, int kv,
-                                          int beam_base, int quarter, int B) {
+                                          int u, int n_q, int Hq, int G, int kv, int beam_base, int quarter,
+                                          float* ch_y, const uint32_t* ch_off) {
     constexpr uint32_t SLOT = 32 * D * 4;
     constexpr int CPR = D / 4;                          // 16-byte chunks per fp32 row
     constexpr int CPO = D / 8;                          // 16-byte chunks per bf16 row
     unsigned char* ring = smem_raw + ring_off;
     // this block's own slot is never written remotely: bf16 output staging [32][D] + per-lane scratch
     unsigned char* stage = ring + (size_t)(ob * ns + me) * SLOT;
-    float* wgt = reinterpret_cast<float*>(stage + 32 * D * 2);          // [16][32]: split weights 0..7, chain 8..15
-    uint32_t* voff = reinterpret_cast<uint32_t*>(wgt + 16 * 32);          // [8][32]: element offset of the V row
+    float* wgt = reinterpret_cast<float*>(stage + 32 * D * 2);          // [8][32]: weights of the other splits
     const int r = quarter * 32 + lane;
-    const int i = beam_base + r / G, g = r % G;
+    const int i = beam_base + r / G;
     const bool live = i < n_q;
     const int level = fa.level;
-    const size_t level_stride = (size_t)B * fa.Wmax * Hkv * D;
     tc_fence_after();
-
-    // ---- chain scores (log2 units) -> wgt[8 + t], row offsets -> voff[t] ----------------------------------
     float m_all = has ? m_own : -INFINITY;
-    if (level > 0) {
-        uint4 qv[D / 8];
-        const uint4* qp = reinterpret_cast<const uint4*>(fa.q + (((size_t)u * n_q + (live ? i : 0)) * Hq + kv * G + g) * D);
-#pragma unroll
-        for (int c = 0; c < D / 8; ++c) qv[c] = __ldg(qp + c);
-#pragma unroll 1
-        for (int t = 0; t < level; ++t) {
-            int a = __ldg(fa.anc + ((size_t)u * fa.Wmax + (live ? i : 0)) * fa.d + t);
-            a = min(max(a, 0), fa.Wmax - 1);            // memory safety on garbage input
-            const size_t off = (size_t)t * level_stride + (((size_t)u * fa.Wmax + a) * Hkv + kv) * D;
-            const uint4* kp = reinterpret_cast<const uint4*>(fa.ks + off);
-            float dot = 0.f;
-#pragma unroll
-            for (int c = 0; c < D / 8; ++c) {
-                const uint4 kk = __ldg(kp + c);
-                const uint32_t qa[4] = {qv[c].x, qv[c].y, qv[c].z, qv[c].w}, ka[4] = {kk.x, kk.y, kk.z, kk.w};
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    dot = fmaf(__uint_as_float(qa[e] << 16), __uint_as_float(ka[e] << 16), dot);
-                    dot = fmaf(__uint_as_float(qa[e] & 0xffff0000u), __uint_as_float(ka[e] & 0xffff0000u), dot);
-                }
-            }
-            const float yt = dot * scale_log2;
-            wgt[(8 + t) * 32 + lane] = yt;
-            voff[t * 32 + lane] = (uint32_t)off;        // suffix buffers are far below 2^32 elements
-            m_all = fmaxf(m_all, yt);
-        }
-    }
+    if (live)
+        for (int t = 0; t < level; ++t) m_all = fmaxf(m_all, ch_y[t]);  // chain scores (log2 units), from the prologue
     // ---- log-sum-exp weights over {own split, delivered splits, chain} ------------------------------------
 #pragma unroll 1
     for (int sidx = 0; sidx < ns; ++sidx)
@@ -286,8 +289,8 @@ __device__ __noinline__ void fused_finish(const FusedArgs& fa, unsigned char* sm
     }
 #pragma unroll 1
     for (int t = 0; t < level; ++t) {
-        const float e = (any && live) ? fast_exp2(wgt[(8 + t) * 32 + lane] - m_all) : 0.f;
-        wgt[(8 + t) * 32 + lane] = e;
+        const float e = (any && live) ? fast_exp2(ch_y[t] - m_all) : 0.f;
+        ch_y[t] = e;                                    // score -> weight, in place
         denom += e;
     }
     const float inv = denom > 0.f ? 1.0f / denom : 0.f;
@@ -316,9 +319,9 @@ __device__ __noinline__ void fused_finish(const FusedArgs& fa, unsigned char* sm
             }
         }
 #pragma unroll 1
-        for (int t = 0; t < level; ++t) {
-            const float e = wgt[(8 + t) * 32 + lane];
-            const uint4* vp = reinterpret_cast<const uint4*>(fa.vs + voff[t * 32 + lane]) + c * 4;
+        for (int t = 0; t < (live ? level : 0); ++t) {
+            const float e = ch_y[t];
+            const uint4* vp = reinterpret_cast<const uint4*>(fa.vs + ch_off[t]) + c * 4;
 #pragma unroll
             for (int k4 = 0; k4 < 4; ++k4) {
                 const uint4 vv = __ldg(vp + k4);
@@ -344,14 +347,13 @@ __device__ __noinline__ void fused_finish(const FusedArgs& fa, unsigned char* sm
     }
     __syncwarp();
     const size_t row_base = (size_t)u * n_q * Hq + kv * G;
-#pragma unroll 1
+#pragma unroll 4
     for (int idx = lane; idx < 32 * CPO; idx += 32) {
         const int l2 = idx / CPO, ch = idx % CPO;
         const int r2 = quarter * 32 + l2;
         const int i2 = beam_base + r2 / G, g2 = r2 % G;
-        if (i2 < n_q)
-            *reinterpret_cast<uint4*>(fa.out + (row_base + (size_t)i2 * Hq + g2) * D + ch * 8) =
-                *reinterpret_cast<const uint4*>(stage + (size_t)l2 * D * 2 + ((ch ^ (l2 & (CPO - 1))) * 16));
+        const uint4 v = *reinterpret_cast<const uint4*>(stage + (size_t)l2 * D * 2 + ((ch ^ (l2 & (CPO - 1))) * 16));
+        if (i2 < n_q) *reinterpret_cast<uint4*>(fa.out + (row_base + (size_t)i2 * Hq + g2) * D + ch * 8) = v;
     }
 }
 
@@ -365,10 +367,15 @@ __global__ void __launch_bounds__(kThreadsTC, 1)
 prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                  const __grid_constant__ CUtensorMap tm_v, const int32_t* __restrict__ cu,
                  float* __restrict__ pm, float* __restrict__ pl, float* __restrict__ po, int B, int n_q,
-                 int Hq, int Hkv, int G, int n_splits, float scale_log2, const FusedArgs fa) {
+                 int Hq, int Hkv, int G, int n_splits, float scale_log2, int parity, const FusedArgs fa) {
+    // Two TMEM accumulator sets (S_t/P_t, O_t), t = 0, 1, each served by its own softmax warpgroup:
+    //   pair mode   (parity = 0): the CTA owns Q tiles 2x and 2x+1; set t = Q tile t; both see every KV tile.
+    //   parity mode (parity = 1): the CTA owns ONE Q tile; set t = the KV tiles of parity t (two independent
+    //                             partial softmaxes over the same rows, merged inside the CTA at the end).
+    // Parity mode doubles the CTA count for the same work -- it is used when pair mode would leave SMs idle.
     using C = TcCfg<D>;
     constexpr int NS = C::NS;
-    const int pair = blockIdx.x;                         // Q tiles 2*pair and 2*pair + 1
+    const int tile0 = parity ? blockIdx.x : 2 * blockIdx.x;  // first (or only) Q tile of this CTA
     // FUSED: the splits of one KV head are adjacent in y (cluster dims (1, n_splits, 1))
     const int kv = FUSED ? blockIdx.y / n_splits : blockIdx.y % Hkv;
     const int split = FUSED ? blockIdx.y % n_splits : blockIdx.y / Hkv;
@@ -384,15 +391,16 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     const int n_tiles = r1 > r0 ? (r1 - r0 + BN - 1) / BN : 0;
     const int beams_per_tile = BM / G;
     const int M = n_q * G;
-    const bool two = M > (2 * pair + 1) * BM;            // does the second Q tile hold any live row?
+    const bool two = !parity && M > (tile0 + 1) * BM;    // pair mode: does the second Q tile hold any live row?
+    const bool both = parity || two;                     // are both accumulator sets in use?
     const size_t split_stride = (size_t)B * n_q * Hq;
 
     if (!FUSED && n_tiles == 0) {  // empty split: (m, l, o) = (-inf, 0, 0), reading R18
         if (warp >= 2) {
             const int t = (warp - 2) >> 2;
             const int r = (threadIdx.x - 64) & 127;
-            const int i = (2 * pair + t) * beams_per_tile + r / G, g = r % G;
-            if (i < n_q) {
+            const int i = (tile0 + (parity ? 0 : t)) * beams_per_tile + r / G, g = r % G;
+            if (i < n_q && !(parity && t == 1)) {
                 const size_t row = split * split_stride + ((size_t)u * n_q + i) * Hq + kv * G + g;
                 pm[row] = -INFINITY; pl[row] = 0.f;
                 float4* o4 = reinterpret_cast<float4*>(po + row * D);
@@ -420,14 +428,26 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
 
     // Warp 0 lane 0 initialises the barriers and immediately starts the first TMA loads: they only need
     // the barriers, not TMEM, so the HBM latency of Q / K_0 / V_0 ... overlaps the TMEM allocation.
+    // The n-th tile through the ring, in the order the tensor pipe consumes them.
+    //   pair:   K_0 V_0 K_1 V_1 ...                      n_k(j) = 2j,  n_v(j) = 2j + 1
+    //   parity: K_0 K_1 V_0 K_2 V_1 K_3 ... V_{nt-2} V_{nt-1}   n_k(x) = x < 2 ? x : 2x - 1,
+    //                                                    n_v(x) = x == nt - 1 ? 2x + 1 : 2x + 2
     int n_issued = 0;
-    auto issue_kv = [&](int n) {                         // n = 2j: K_j, n = 2j + 1: V_j
+    auto seq_k = [&](int x) { return parity ? (x < 2 ? x : 2 * x - 1) : 2 * x; };
+    auto seq_v = [&](int x) { return parity ? (x == n_tiles - 1 ? 2 * x + 1 : 2 * x + 2) : 2 * x + 1; };
+    auto issue_kv = [&](int n) {
+        bool is_v; int x;
+        if (!parity) { is_v = n & 1; x = n >> 1; }
+        else if (n_tiles == 1) { is_v = n == 1; x = 0; }
+        else if (n < 2) { is_v = false; x = n; }
+        else if (n >= 2 * n_tiles - 2) { is_v = true; x = n - n_tiles; }
+        else { is_v = !(n & 1); x = is_v ? (n - 2) >> 1 : ((n - 3) >> 1) + 2; }
         const int s = n % NS;
-        const int row = row_begin + r0 + (n >> 1) * BN;
+        const int row = row_begin + r0 + x * BN;
         mbar_expect_tx(bar_full + 8 * s, C::TILE_BYTES);
 #pragma unroll
         for (int bx = 0; bx < C::BOXES; ++bx)
-            tma_load_3d(sKV + s * C::TILE_BYTES + bx * (BN * 128), (n & 1) ? &tm_v : &tm_k, bar_full + 8 * s,
+            tma_load_3d(sKV + s * C::TILE_BYTES + bx * (BN * 128), is_v ? &tm_v : &tm_k, bar_full + 8 * s,
                         bx * 64, kv, row);
     };
     if (threadIdx.x == 0) {
@@ -440,7 +460,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
         mbar_init(bar_done, 1);
         fence_barrier_init();
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        const int beam0 = u * n_q + 2 * pair * beams_per_tile;
+        const int beam0 = u * n_q + tile0 * beams_per_tile;
         if (n_tiles > 0) {                               // (a fused CTA with an empty split loads nothing)
             mbar_expect_tx(bar_q, (two ? 2 : 1) * C::TILE_BYTES);
             for (int t = 0; t < (two ? 2 : 1); ++t)
@@ -461,12 +481,19 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     const int t = (warp - 2) >> 2;                      // Q tile (= warpgroup) of this warp
     const int quarter = warp & 3;                       // TMEM lane quarter this warp may access
     const int r = quarter * 32 + lane;                  // query row inside the Q tile
-    const int i = (2 * pair + t) * beams_per_tile + r / G, g = r % G;
+    const int i = (tile0 + (parity ? 0 : t)) * beams_per_tile + r / G, g = r % G;
     const bool live = warp >= 2 && i < n_q;
     const bool warp_live = __any_sync(0xffffffffu, live);
     const uint32_t lane_addr = tmem + ((uint32_t)(quarter * 32) << 16);
     const uint32_t aO = lane_addr + C::COL_O + t * 128;
     float m_ref = -INFINITY, l_sum = 0.f;               // m_ref in log2 units of the scaled score
+    // fused mode: who finishes this warp's 32-row block (see the tail below)
+    const bool mine = FUSED && warp >= 2 && (t == 0 || two) && warp_live;  // the block has live rows
+    const int blk = t * 4 + quarter;                    // 32-row block of the CTA's (up to) 256 rows
+    const int owner = blk % n_splits, ob = blk / n_splits;                 // cluster rank that finishes it
+    const uint32_t me = (FUSED && n_splits > 1) ? cluster_rank() : 0u;
+    float ch_y[8];                                      // chain scores, later weights (fused mode)
+    uint32_t ch_off[8];                                 // chain row offsets in the suffix buffers
 
     if (warp == 0) {
         // ===================== TMA producer (rest of the stream) =====================
@@ -487,7 +514,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
 #pragma unroll
                 for (int k = 0; k < D / 16; ++k) {
                     const uint32_t off = (k / 4) * (BM * 128) + (k % 4) * 32;  // box, then 32 B per K=16 step
-                    umma_ss(d_tmem, smem_desc(sQ + t * C::TILE_BYTES + off, 16, 1024),
+                    umma_ss(d_tmem, smem_desc(sQ + (parity ? 0 : t) * C::TILE_BYTES + off, 16, 1024),
                             smem_desc(sKV + s * C::TILE_BYTES + off, 16, 1024), idesc_s, k > 0 ? 1u : 0u);
                 }
                 umma_commit(bar_sfull + 8 * t);
@@ -502,51 +529,82 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
             };
             auto slot_of = [&](int n) { return n % NS; };
             auto wait_full = [&](int n) { mbar_wait(bar_full + 8 * slot_of(n), (uint32_t)((n / NS) & 1)); tc_fence_after(); };
-            const int nt = two ? 2 : 1;
             mbar_wait(bar_q, 0);
-            wait_full(0);
-            for (int t = 0; t < nt; ++t) issue_qk(t, slot_of(0));
-            umma_commit(bar_empty + 8 * slot_of(0));
-            for (int j = 0; j < n_tiles; ++j) {
-                const bool more = j + 1 < n_tiles;
-                wait_full(2 * j + 1);                    // V_j
-                if (more) wait_full(2 * j + 2);          // K_{j+1}
-                for (int t = 0; t < nt; ++t) {
-                    mbar_wait(bar_pfull + 8 * t, (uint32_t)(j & 1));
-                    tc_fence_after();
-                    issue_pv(t, slot_of(2 * j + 1), j > 0);
-                    if (more) issue_qk(t, slot_of(2 * j + 2));
+            if (!parity) {
+                // PV0_j, QK0_{j+1}, PV1_j, QK1_{j+1}: one Q tile's MMAs run while the other's softmax does
+                const int nt = two ? 2 : 1;
+                wait_full(0);
+                for (int t = 0; t < nt; ++t) issue_qk(t, slot_of(0));
+                umma_commit(bar_empty + 8 * slot_of(0));
+                for (int j = 0; j < n_tiles; ++j) {
+                    const bool more = j + 1 < n_tiles;
+                    wait_full(2 * j + 1);                    // V_j
+                    if (more) wait_full(2 * j + 2);          // K_{j+1}
+                    for (int t = 0; t < nt; ++t) {
+                        mbar_wait(bar_pfull + 8 * t, (uint32_t)(j & 1));
+                        tc_fence_after();
+                        issue_pv(t, slot_of(2 * j + 1), j > 0);
+                        if (more) issue_qk(t, slot_of(2 * j + 2));
+                    }
+                    umma_commit(bar_empty + 8 * slot_of(2 * j + 1));
+                    if (more) umma_commit(bar_empty + 8 * slot_of(2 * j + 2));
                 }
-                umma_commit(bar_empty + 8 * slot_of(2 * j + 1));
-                if (more) umma_commit(bar_empty + 8 * slot_of(2 * j + 2));
+            } else {
+                // KV tile x belongs to accumulator set x & 1: PV_t(x), QK_t(x + 2), alternating t
+                for (int x = 0; x < min(2, n_tiles); ++x) {
+                    wait_full(seq_k(x));
+                    issue_qk(x, slot_of(seq_k(x)));
+                    umma_commit(bar_empty + 8 * slot_of(seq_k(x)));
+                }
+                for (int x = 0; x < n_tiles; ++x) {
+                    const int t = x & 1;
+                    wait_full(seq_v(x));
+                    mbar_wait(bar_pfull + 8 * t, (uint32_t)((x >> 1) & 1));
+                    tc_fence_after();
+                    issue_pv(t, slot_of(seq_v(x)), x >= 2);
+                    umma_commit(bar_empty + 8 * slot_of(seq_v(x)));
+                    if (x + 2 < n_tiles) {
+                        wait_full(seq_k(x + 2));
+                        issue_qk(t, slot_of(seq_k(x + 2)));
+                        umma_commit(bar_empty + 8 * slot_of(seq_k(x + 2)));
+                    }
+                }
             }
             umma_commit(bar_done);
         }
     } else {
         // ===================== softmax / correction / epilogue =====================
-        if (t == 0 || two) {
+        if (FUSED && mine && owner == (int)me && live && fa.level > 0)  // overlaps the first K/V tiles' flight
+            chain_scores<D>(fa, scale_log2, u, i, kv * G + g, kv, n_q, Hq, Hkv, B, ch_y, ch_off);
+        if (t == 0 || both) {
             const uint32_t aS = lane_addr + C::COL_S + t * BN;
-            for (int j = 0; j < n_tiles; ++j) {
+            const int my_tiles = parity ? (n_tiles - t + 1) / 2 : n_tiles;  // KV tiles of this accumulator set
+            for (int j = 0; j < my_tiles; ++j) {
                 mbar_wait(bar_sfull + 8 * t, (uint32_t)(j & 1));
                 __syncwarp();
                 if (warp_live) {                        // warps without live rows only keep the barrier count
                     tc_fence_after();
-                    const int valid = min(BN, r1 - (r0 + j * BN));  // columns of this tile inside the split
-                    // pass 1 over the S row: maximum
+                    const int x = parity ? 2 * j + t : j;            // KV tile of the split
+                    const int valid = min(BN, r1 - (r0 + x * BN));   // columns of this tile inside the split
+                    // the whole S row (128 fp32) into registers with one wait, then its maximum
+                    uint32_t sr[4][32];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) tmem_ld32(aS + c * 32, sr[c]);
+                    tmem_wait_ld();
                     float tmax = -INFINITY;
+                    if (valid >= BN) {
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        uint32_t sr[32];
-                        tmem_ld32(aS + c * 32, sr);
-                        tmem_wait_ld();
-                        if (valid >= BN) {
+                        for (int c = 0; c < 4; ++c)
 #pragma unroll
-                            for (int x = 0; x < 32; ++x) tmax = fmaxf(tmax, __uint_as_float(sr[x]));
-                        } else {
+                            for (int x = 0; x < 32; ++x) tmax = fmaxf(tmax, __uint_as_float(sr[c][x]));
+                    } else {
 #pragma unroll
-                            for (int x = 0; x < 32; ++x)
-                                if (c * 32 + x < valid) tmax = fmaxf(tmax, __uint_as_float(sr[x]));
-                        }
+                        for (int c = 0; c < 4; ++c)
+#pragma unroll
+                            for (int x = 0; x < 32; ++x) {
+                                if (c * 32 + x >= valid) sr[c][x] = 0xff800000u;  // -inf: exp2 gives exactly 0
+                                tmax = fmaxf(tmax, __uint_as_float(sr[c][x]));
+                            }
                     }
                     tmax *= scale_log2;
                     // lazy rescale: keep the reference maximum unless the row maximum grew by > 2^8
@@ -569,23 +627,17 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                         l_sum *= alpha;
                     }
                     m_ref = m_new;
-                    // pass 2: P = exp2(s * scale - m_ref) as bf16, written over S in place (P chunk c covers
-                    // columns [16c, 16c+16), all of them already consumed)
+                    // P = exp2(s * scale - m_ref) as bf16, written over S in place (P chunk c covers columns
+                    // [16c, 16c+16) of the S region, whose contents are already in registers)
                     const float neg_m = -m_ref;
                     float psum = 0.f;
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
-                        uint32_t sr[32], pk[16];
-                        tmem_ld32(aS + c * 32, sr);
-                        tmem_wait_ld();
+                        uint32_t pk[16];
 #pragma unroll
                         for (int x = 0; x < 32; x += 2) {
-                            float p0 = fast_exp2(fmaf(__uint_as_float(sr[x]), scale_log2, neg_m));
-                            float p1 = fast_exp2(fmaf(__uint_as_float(sr[x + 1]), scale_log2, neg_m));
-                            if (valid < BN) {
-                                if (c * 32 + x >= valid) p0 = 0.f;
-                                if (c * 32 + x + 1 >= valid) p1 = 0.f;
-                            }
+                            const float p0 = fast_exp2(fmaf(__uint_as_float(sr[c][x]), scale_log2, neg_m));
+                            const float p1 = fast_exp2(fmaf(__uint_as_float(sr[c][x + 1]), scale_log2, neg_m));
                             psum += p0 + p1;
                             const __nv_bfloat162 h = __floats2bfloat162_rn(p0, p1);  // element 2x in the low half
                             pk[x >> 1] = *reinterpret_cast<const uint32_t*>(&h);
@@ -601,13 +653,65 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
             // ---- epilogue: O row -> partials ----
             if (n_tiles > 0) mbar_wait(bar_done, 0);
             __syncwarp();
-            if (!FUSED && warp_live) {
+            if (parity) {
+                // ---- parity mode: fold accumulator set 1 (odd KV tiles) into set 0 inside the CTA ----
+                // set 1's rows go through the (now idle) K/V ring: block `quarter`, chunks XOR-swizzled by row
+                constexpr int CPRm = D / 4;
+                unsigned char* ring = smem_raw + (sKV - smem_u32(smem_raw));
+                float* mrow = reinterpret_cast<float*>(ring) + (size_t)quarter * 32 * D + lane * D;
+                float2* mml = reinterpret_cast<float2*>(ring + 8 * 32 * D * 4) + quarter * 32 + lane;
+                if (t == 1 && warp_live) {
+                    tc_fence_after();
+                    *mml = make_float2(m_ref, l_sum);
+                    if (my_tiles > 0) {
+#pragma unroll
+                        for (int c = 0; c < D / 32; ++c) {
+                            uint32_t o[32];
+                            tmem_ld32(aO + c * 32, o);
+                            tmem_wait_ld();
+#pragma unroll
+                            for (int x = 0; x < 32; x += 4)
+                                *reinterpret_cast<float4*>(mrow + (((c * 8 + (x >> 2)) ^ (lane & (CPRm - 1))) * 4)) =
+                                    make_float4(__uint_as_float(o[x]), __uint_as_float(o[x + 1]),
+                                                __uint_as_float(o[x + 2]), __uint_as_float(o[x + 3]));
+                        }
+                    }
+                }
+                asm volatile("bar.sync 2, 256;" ::: "memory");  // the two softmax warpgroups
+                if (t == 0 && warp_live) {
+                    const float2 ml = *mml;
+                    if (ml.x > -INFINITY) {             // set 1 saw at least one KV tile (so did set 0)
+                        tc_fence_after();
+                        const float m = fmaxf(m_ref, ml.x);
+                        const float a0 = fast_exp2(m_ref - m), a1 = fast_exp2(ml.x - m);
+#pragma unroll
+                        for (int c = 0; c < D / 32; ++c) {
+                            uint32_t o[32];
+                            tmem_ld32(aO + c * 32, o);
+                            tmem_wait_ld();
+#pragma unroll
+                            for (int x = 0; x < 32; x += 4) {
+                                const float4 v = *reinterpret_cast<const float4*>(mrow + (((c * 8 + (x >> 2)) ^ (lane & (CPRm - 1))) * 4));
+                                o[x] = __float_as_uint(fmaf(a1, v.x, a0 * __uint_as_float(o[x])));
+                                o[x + 1] = __float_as_uint(fmaf(a1, v.y, a0 * __uint_as_float(o[x + 1])));
+                                o[x + 2] = __float_as_uint(fmaf(a1, v.z, a0 * __uint_as_float(o[x + 2])));
+                                o[x + 3] = __float_as_uint(fmaf(a1, v.w, a0 * __uint_as_float(o[x + 3])));
+                            }
+                            tmem_st32(aO + c * 32, o);
+                        }
+                        tmem_wait_st();
+                        l_sum = a0 * l_sum + a1 * ml.y;
+                        m_ref = m;
+                    }
+                }
+            }
+            if (!FUSED && warp_live && !(parity && t == 1)) {
                 tc_fence_after();
                 // Each thread owns one O row (512 B), so direct stores would scatter 16-byte pieces over 32
                 // rows per instruction (measured: 5.5 us for 17 MB).  Stage the warp's 32 rows in the (now
                 // idle) K/V ring, 16-byte chunks XOR-swizzled by row, then write whole rows coalesced.
                 constexpr int CPR = D / 4;              // 16-byte chunks per row
-                float* stage = reinterpret_cast<float*>(smem_raw + (sKV - smem_u32(smem_raw))) + (size_t)(warp - 2) * 32 * D;
+                float* stage = reinterpret_cast<float*>(smem_raw + (sKV - smem_u32(smem_raw))) + (size_t)(t * 4 + quarter) * 32 * D;
 #pragma unroll
                 for (int c = 0; c < D / 32; ++c) {
                     uint32_t o[32];
@@ -627,7 +731,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 for (int idx = lane; idx < 32 * CPR; idx += 32) {
                     const int l2 = idx / CPR, ch = idx % CPR;
                     const int r2 = quarter * 32 + l2;
-                    const int i2 = (2 * pair + t) * beams_per_tile + r2 / G, g2 = r2 % G;
+                    const int i2 = (tile0 + (parity ? 0 : t)) * beams_per_tile + r2 / G, g2 = r2 % G;
                     if (i2 < n_q)
                         *reinterpret_cast<float4*>(po + (row_base + (size_t)i2 * Hq + g2) * D + ch * 4) =
                             *reinterpret_cast<const float4*>(stage + l2 * D + ((ch ^ (l2 & (CPR - 1))) * 4));
@@ -637,10 +741,6 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
         }
     }
     if constexpr (FUSED) {
-        const bool mine = warp >= 2 && (t == 0 || two) && warp_live;  // this warp's 32-row block has live rows
-        const int blk = t * 4 + quarter;                               // 32-row block of the 256-row pair
-        const int owner = blk % n_splits, ob = blk / n_splits;         // cluster rank that finishes it
-        const uint32_t me = n_splits > 1 ? cluster_rank() : 0u;
         constexpr uint32_t SLOT = 32 * D * 4;                          // one block of fp32 O rows
         const uint32_t ml_base = sKV + 8 * SLOT;                       // (m, l) pairs: [slot][32][2]
         // B1: every CTA of the cluster is done with its K/V ring, which now becomes the exchange buffer
@@ -670,7 +770,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
         if (n_splits > 1) cluster_sync_all();                          // B2: all partial rows delivered
         if (mine && owner == (int)me)
             fused_finish<D>(fa, smem_raw, sKV - smem_u32(smem_raw), ob, (int)me, n_splits, lane, aO, n_tiles > 0, m_ref,
-                            l_sum, scale_log2, u, n_q, Hq, Hkv, G, kv, (2 * pair + t) * beams_per_tile, quarter, B);
+                            l_sum, u, n_q, Hq, G, kv, (tile0 + (parity ? 0 : t)) * beams_per_tile, quarter, ch_y, ch_off);
         tc_fence_before();
     }
     __syncthreads();
@@ -723,9 +823,11 @@ int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const 
         attr_done = true;
     }
     const int M = n_q * p.G;
-    dim3 grid((M + 2 * BM - 1) / (2 * BM), p.Hkv * n_splits, p.B);  // one CTA per pair of Q tiles
+    const int parity = prefix_tc_parity(p, n_q, n_splits) ? 1 : 0;
+    const int rows_per_cta = parity ? BM : 2 * BM;                  // one Q tile, or a pair of them
+    dim3 grid((M + rows_per_cta - 1) / rows_per_cta, p.Hkv * n_splits, p.B);
     prefix_tc_kernel<D, false><<<grid, kThreadsTC, TcCfg<D>::SMEM_BYTES, st>>>(
-        tq, tk, tv, cu, pm, pl, po, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits, p.scale * kLog2e, FusedArgs{});
+        tq, tk, tv, cu, pm, pl, po, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits, p.scale * kLog2e, parity, FusedArgs{});
     STARK_LAUNCH_CHECK();
     return STARK_OK;
 }
@@ -741,8 +843,10 @@ int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, 
         attr_done = true;
     }
     const int M = n_q * p.G;
+    const int parity = prefix_tc_parity(p, n_q, n_splits) ? 1 : 0;
+    const int rows_per_cta = parity ? BM : 2 * BM;
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((M + 2 * BM - 1) / (2 * BM), p.Hkv * n_splits, p.B);
+    cfg.gridDim = dim3((M + rows_per_cta - 1) / rows_per_cta, p.Hkv * n_splits, p.B);
     cfg.blockDim = dim3(kThreadsTC);
     cfg.dynamicSmemBytes = TcCfg<D>::SMEM_BYTES;
     cfg.stream = st;
@@ -752,11 +856,19 @@ int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, 
     cfg.attrs = at; cfg.numAttrs = 1;
     STARK_CUDA_TRY(cudaLaunchKernelEx(&cfg, prefix_tc_kernel<D, true>, tq, tk, tv, cu, (float*)nullptr,
                                       (float*)nullptr, (float*)nullptr, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits,
-                                      p.scale * kLog2e, fa));
+                                      p.scale * kLog2e, parity, fa));
     return STARK_OK;
 }
 
 }  // namespace
+
+// Parity mode (one Q tile per CTA, KV tiles alternating between the two accumulator sets) whenever its
+// doubled CTA count still fits the GPU in one wave; pair mode (K/V staged once per 256 rows) otherwise.
+bool prefix_tc_parity(const Dims& p, int n_q, int n_splits) {
+    const int sms = num_sms() > 0 ? num_sms() : 148;
+    const long long tiles_m = ((long long)n_q * p.G + BM - 1) / BM;
+    return tiles_m * p.Hkv * p.B * n_splits <= sms;
+}
 
 bool prefix_tc_supported(const Dims& p, int dtype, int n_q) {
     if (dtype != STARK_BF16) return false;
