@@ -42,6 +42,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="launch eagerly instead of replaying CUDA graphs")
     ap.add_argument("--sets", type=int, default=0, help="rotating input sets (0 = enough to exceed L2)")
+    ap.add_argument("--calibrate", action="store_true",
+                    help="print launch-floor / cold-stream floors of this GPU (DESIGN.md section 7) and exit")
     return ap.parse_args()
 
 
@@ -212,6 +214,44 @@ def oracle_sample(cfg, n_users, seed=0):
     return time.perf_counter() - t0, n_sids, threads
 
 
+def shard_seed(rank: int, r: int) -> int:
+    """Seed of rotating input set r on rank `rank`: every rank decodes its own users (replicas, no collective)."""
+    return rank * 1000 + r
+
+
+def max_over_ranks(ms: float, dist=None, device=None) -> float:
+    """Whole-job time of a weak-scaling replica run = the slowest rank's device time."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, sids_per_pass: int, ms_per_step: float) -> float:
+    """SIDs/s of all ranks together (each rank finishes sids_per_pass SIDs per step)."""
+    return world * sids_per_pass / (ms_per_step * 1e-3)
+
+
+def run_calibrate():
+    """Launch floor and plain cold-stream floors (one graph of 24 launches rotating over buffers > L2)."""
+    import torch
+    from paper_2607_04068_b200 import binding as sb
+    sb.lib()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    sink = torch.zeros(1, dtype=torch.int32, device=dev)
+    bufs = [torch.zeros(64 << 20, dtype=torch.uint8, device=dev) for _ in range(8)]   # 512 MB rotation
+    out = {"empty_kernel_us": time_graph_loop(torch, [sb.stark_calib_empty], 480)}
+    for mb in (1, 4, 19, 34, 46, 64):
+        fns = [(lambda b=b, mb=mb: sb.stark_calib_stream_read(b, mb << 20, sink)) for b in bufs]
+        us = time_graph_loop(torch, fns, 480)
+        note = "L2-resident (8 x %d MB < L2)" % mb if 8 * mb < 126 else "cold"
+        out[f"stream_read_{mb}MB"] = {"us": round(us, 2), "GBps": round((mb << 20) / us * 1e-3, 1), "state": note}
+    print(json.dumps({"calibration": out}), flush=True)
+
+
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -262,11 +302,11 @@ def run_stark(args, cfg):
     sb.lib()
 
     # ---- inputs: R rotating sets so that consecutive passes never hit a warm L2 ----------------
-    h0 = host_inputs(cfg, seed=rank * 1000)
+    h0 = host_inputs(cfg, seed=shard_seed(rank, 0))
     set_bytes = sum(a.nbytes // (2 if cfg.dtype == "bf16" else 1) for a in [h0["K"], h0["V"], *h0["q"], *h0["k"], *h0["v"]]) \
         + sum(a.nbytes for a in h0["lg"])
     R = args.sets or int(min(16, max(2, -(-2 * L2_BYTES // set_bytes))))
-    hosts = [h0] + [host_inputs(cfg, seed=rank * 1000 + r) for r in range(1, R)]
+    hosts = [h0] + [host_inputs(cfg, seed=shard_seed(rank, r)) for r in range(1, R)]
     passes = [make_pass(cfg, h, dev) for h in hosts]
     lens = np.diff(h0["cu"])
     widths = wl.beam_widths(cfg)
@@ -307,10 +347,7 @@ def run_stark(args, cfg):
     barrier()
     sampler.active = False
     ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist if world > 1 else None, dev)
     if len(sampler.samples) < 5:           # short timed region: sample a longer replay of the same work
         sampler.active = True
         t_end = time.time() + 0.3
@@ -324,7 +361,7 @@ def run_stark(args, cfg):
         sampler.active = False
     sampler.stop_flag = True
     ms_per_step = ms / args.steps
-    value = world * sids_per_pass / (ms_per_step * 1e-3)
+    value = whole_job_value(world, sids_per_pass, ms_per_step)
     if rank != 0:
         if world > 1:
             dist.barrier()
@@ -441,6 +478,8 @@ def run_stark(args, cfg):
 
 def main():
     args = parse_args()
+    if args.calibrate:
+        return run_calibrate()
     cfg = wl.get_config(args.workload)
     if args.impl == "reference":
         run_reference(args, cfg)

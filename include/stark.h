@@ -256,6 +256,18 @@ size_t stark_suffix_bytes(const stark_shape_t* shape);
 /* Bytes of anc: 2*B*Wmax*d*4. */
 size_t stark_anc_bytes(const stark_shape_t* shape);
 
+/* ---------------------------------------------------------------------------
+ * Measurement aids (used by `bench.py --calibrate`; not part of the method).
+ * stark_calib_empty: launches an empty kernel -- the launch floor.
+ * stark_calib_stream_read: a plain grid-stride 16-byte read of `bytes` bytes of
+ * device memory `src` (148*8 CTAs of 256 threads, 4 loads in flight per thread)
+ * -- what a trivial HBM-bound kernel of that size achieves, launch and ramp
+ * included; sink must point to 4 writable device bytes (never written unless
+ * the data XORs to a magic value).  Errors: INVALID_ARG, CUDA.
+ */
+int stark_calib_empty(void* stream);
+int stark_calib_stream_read(const void* src, size_t bytes, void* sink, void* stream);
+
 int stark_version(void);
 /* Static string describing a stark_status_t. */
 const char* stark_status_string(int status);

@@ -221,6 +221,19 @@ int stark_decode_attn(const stark_shape_t* shape, const void* q, int n_q, int le
                                (cudaStream_t)stream);
 }
 
+int stark_calib_empty(void* stream) {
+    const int rc = check_device();
+    if (rc != STARK_OK) return rc;
+    return launch_calib(nullptr, 0, nullptr, (cudaStream_t)stream);
+}
+
+int stark_calib_stream_read(const void* src, size_t bytes, void* sink, void* stream) {
+    if (!src || !sink || bytes < 16) return STARK_ERR_INVALID_ARG;
+    const int rc = check_device();
+    if (rc != STARK_OK) return rc;
+    return launch_calib(src, bytes, sink, (cudaStream_t)stream);
+}
+
 int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_in, int C, int W_out,
                     float* out_score, int32_t* out_parent, int32_t* out_code, void* ws, size_t ws_bytes,
                     void* stream) {
