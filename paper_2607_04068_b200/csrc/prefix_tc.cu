@@ -46,7 +46,8 @@ namespace {
 
 constexpr int BM = 128;          // query rows per Q tile = MMA M (two Q tiles per CTA)
 constexpr int BN = 128;          // KV rows per tile      = MMA N of S, K-extent of P V
-constexpr int kThreadsTC = 320;  // TMA warp + MMA warp + 2 softmax warpgroups
+constexpr int kThreadsTC = 384;  // warpgroup 0: TMA warp, MMA warp (2 idle); warpgroups 1, 2: softmax
+constexpr int kFirstSoftmaxWarp = 4;
 constexpr int kSoftmaxThreads = 128;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units
 
@@ -218,7 +219,7 @@ template <int D> struct TcCfg {
 // scaled score, and the element offsets of the chain's rows in the suffix buffers.  Independent of the prefix,
 // so the fused kernel runs it while the first K/V tiles are still in flight.
 template <int D>
-__device__ __noinline__ void chain_scores(const FusedArgs& fa, float scale_log2, int u, int i, int h, int kv, int n_q,
+__device__ __forceinline__ void chain_scores(const FusedArgs& fa, float scale_log2, int u, int i, int h, int kv, int n_q,
                                           int Hq, int Hkv, int B, float* y, uint32_t* off_out) {
     const size_t level_stride = (size_t)B * fa.Wmax * Hkv * D;
     uint4 qv[D / 8];
@@ -253,7 +254,7 @@ __device__ __noinline__ void chain_scores(const FusedArgs& fa, float scale_log2,
 // Runs once per CTA, so it is written for SMALL CODE (rolled loops, per-lane scratch in shared memory): a
 // fully unrolled version was instruction-fetch bound (~100 KB of straight-line code: 16 us).
 template <int D>
-__device__ __noinline__ void fused_finish(const FusedArgs& fa, unsigned char* smem_raw, uint32_t ring_off, int ob, int me,
+__device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char* smem_raw, uint32_t ring_off, int ob, int me,
                                           int ns, int lane, uint32_t aO, bool has, float m_own, float l_own,
                                           int u, int n_q, int Hq, int G, int kv, int beam_base, int quarter,
                                           float* ch_y, const uint32_t* ch_off) {
@@ -396,9 +397,9 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     const size_t split_stride = (size_t)B * n_q * Hq;
 
     if (!FUSED && n_tiles == 0) {  // empty split: (m, l, o) = (-inf, 0, 0), reading R18
-        if (warp >= 2) {
-            const int t = (warp - 2) >> 2;
-            const int r = (threadIdx.x - 64) & 127;
+        if (warp >= kFirstSoftmaxWarp) {
+            const int t = (warp - kFirstSoftmaxWarp) >> 2;
+            const int r = threadIdx.x & 127;
             const int i = (tile0 + (parity ? 0 : t)) * beams_per_tile + r / G, g = r % G;
             if (i < n_q && !(parity && t == 1)) {
                 const size_t row = split * split_stride + ((size_t)u * n_q + i) * Hq + kv * G + g;
@@ -478,24 +479,31 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     const uint32_t tmem = *tmem_slot_ptr;
 
     // identity of a softmax warp (warps 2..9; harmless values for warps 0 and 1)
-    const int t = (warp - 2) >> 2;                      // Q tile (= warpgroup) of this warp
+    const int t = (warp - kFirstSoftmaxWarp) >> 2;      // accumulator set (= warpgroup) of this warp
     const int quarter = warp & 3;                       // TMEM lane quarter this warp may access
     const int r = quarter * 32 + lane;                  // query row inside the Q tile
     const int i = (tile0 + (parity ? 0 : t)) * beams_per_tile + r / G, g = r % G;
-    const bool live = warp >= 2 && i < n_q;
+    const bool live = warp >= kFirstSoftmaxWarp && i < n_q;
     const bool warp_live = __any_sync(0xffffffffu, live);
     const uint32_t lane_addr = tmem + ((uint32_t)(quarter * 32) << 16);
     const uint32_t aO = lane_addr + C::COL_O + t * 128;
     float m_ref = -INFINITY, l_sum = 0.f;               // m_ref in log2 units of the scaled score
     // fused mode: who finishes this warp's 32-row block (see the tail below)
-    const bool mine = FUSED && warp >= 2 && (t == 0 || two) && warp_live;  // the block has live rows
+    const bool mine = FUSED && warp >= kFirstSoftmaxWarp && (t == 0 || two) && warp_live;  // the block has live rows
     const int blk = t * 4 + quarter;                    // 32-row block of the CTA's (up to) 256 rows
     const int owner = blk % n_splits, ob = blk / n_splits;                 // cluster rank that finishes it
     const uint32_t me = (FUSED && n_splits > 1) ? cluster_rank() : 0u;
     float ch_y[8];                                      // chain scores, later weights (fused mode)
     uint32_t ch_off[8];                                 // chain row offsets in the suffix buffers
 
-    if (warp == 0) {
+    // Register budget (setmaxnreg works on whole, aligned warpgroups): warpgroup 0 holds the two single-thread
+    // roles and gives registers back; the softmax warpgroups take them -- a thread keeps its whole S row
+    // (128 fp32) in registers between the row maximum and the exponentials.
+    // (The limits are set at the top of each role's branch, and the fused tail lives inside the softmax
+    // branch: code after a join of the branches would have to fit the smallest budget.)
+    if (warp < kFirstSoftmaxWarp) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        if (warp == 0) {
         // ===================== TMA producer (rest of the stream) =====================
         if (lane == 0) {
             for (int n = n_issued; n < 2 * n_tiles; ++n) {
@@ -503,7 +511,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 issue_kv(n);
             }
         }
-    } else if (warp == 1) {
+        } else if (warp == 1) {
         // ===================== MMA issuer =====================
         if (lane == 0 && n_tiles > 0) {
             constexpr uint32_t idesc_s = instr_desc(BM, BN, 0);
@@ -572,7 +580,14 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
             }
             umma_commit(bar_done);
         }
+        }
+        if (FUSED && n_splits > 1) {                     // the two cluster barriers of the fused tail (B1, B2)
+            __syncwarp();
+            cluster_sync_all();
+            cluster_sync_all();
+        }
     } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
         // ===================== softmax / correction / epilogue =====================
         if (FUSED && mine && owner == (int)me && live && fa.level > 0)  // overlaps the first K/V tiles' flight
             chain_scores<D>(fa, scale_log2, u, i, kv * G + g, kv, n_q, Hq, Hkv, B, ch_y, ch_off);
@@ -591,21 +606,26 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
 #pragma unroll
                     for (int c = 0; c < 4; ++c) tmem_ld32(aS + c * 32, sr[c]);
                     tmem_wait_ld();
-                    float tmax = -INFINITY;
-                    if (valid >= BN) {
+                    if (valid < BN) {
 #pragma unroll
                         for (int c = 0; c < 4; ++c)
 #pragma unroll
-                            for (int x = 0; x < 32; ++x) tmax = fmaxf(tmax, __uint_as_float(sr[c][x]));
-                    } else {
-#pragma unroll
-                        for (int c = 0; c < 4; ++c)
-#pragma unroll
-                            for (int x = 0; x < 32; ++x) {
+                            for (int x = 0; x < 32; ++x)
                                 if (c * 32 + x >= valid) sr[c][x] = 0xff800000u;  // -inf: exp2 gives exactly 0
-                                tmax = fmaxf(tmax, __uint_as_float(sr[c][x]));
-                            }
                     }
+                    // 4 independent running maxima: with two warps per scheduler a single 128-long dependent
+                    // chain (4 cycles per link) would cost as much as the exponentials themselves
+                    float tm0 = -INFINITY, tm1 = -INFINITY, tm2 = -INFINITY, tm3 = -INFINITY;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)
+#pragma unroll
+                        for (int x = 0; x < 32; x += 4) {
+                            tm0 = fmaxf(tm0, __uint_as_float(sr[c][x]));
+                            tm1 = fmaxf(tm1, __uint_as_float(sr[c][x + 1]));
+                            tm2 = fmaxf(tm2, __uint_as_float(sr[c][x + 2]));
+                            tm3 = fmaxf(tm3, __uint_as_float(sr[c][x + 3]));
+                        }
+                    float tmax = fmaxf(fmaxf(tm0, tm1), fmaxf(tm2, tm3));
                     tmax *= scale_log2;
                     // lazy rescale: keep the reference maximum unless the row maximum grew by > 2^8
                     bool grow = false;
@@ -630,7 +650,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                     // P = exp2(s * scale - m_ref) as bf16, written over S in place (P chunk c covers columns
                     // [16c, 16c+16) of the S region, whose contents are already in registers)
                     const float neg_m = -m_ref;
-                    float psum = 0.f;
+                    float ps0 = 0.f, ps1 = 0.f;             // independent partial sums (same reason)
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
                         uint32_t pk[16];
@@ -638,13 +658,13 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                         for (int x = 0; x < 32; x += 2) {
                             const float p0 = fast_exp2(fmaf(__uint_as_float(sr[c][x]), scale_log2, neg_m));
                             const float p1 = fast_exp2(fmaf(__uint_as_float(sr[c][x + 1]), scale_log2, neg_m));
-                            psum += p0 + p1;
+                            ps0 += p0; ps1 += p1;
                             const __nv_bfloat162 h = __floats2bfloat162_rn(p0, p1);  // element 2x in the low half
                             pk[x >> 1] = *reinterpret_cast<const uint32_t*>(&h);
                         }
                         tmem_st16(aS + c * 16, pk);
                     }
-                    l_sum += psum;
+                    l_sum += ps0 + ps1;
                     tmem_wait_st();
                     tc_fence_before();
                 }
@@ -739,39 +759,39 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 tc_fence_before();
             }
         }
-    }
-    if constexpr (FUSED) {
-        constexpr uint32_t SLOT = 32 * D * 4;                          // one block of fp32 O rows
-        const uint32_t ml_base = sKV + 8 * SLOT;                       // (m, l) pairs: [slot][32][2]
-        // B1: every CTA of the cluster is done with its K/V ring, which now becomes the exchange buffer
-        if (n_splits > 1) cluster_sync_all();
-        if (mine && owner != (int)me) {
-            tc_fence_after();
-            const uint32_t slot = (uint32_t)(ob * n_splits) + me;
-            const uint32_t dst = map_to_rank(sKV + slot * SLOT + (uint32_t)lane * D * 4, (uint32_t)owner);
-            constexpr int CPR = D / 4;
+        if constexpr (FUSED) {
+            constexpr uint32_t SLOT = 32 * D * 4;                          // one block of fp32 O rows
+            const uint32_t ml_base = sKV + 8 * SLOT;                       // (m, l) pairs: [slot][32][2]
+            // B1: every CTA of the cluster is done with its K/V ring, which now becomes the exchange buffer
+            if (n_splits > 1) cluster_sync_all();
+            if (mine && owner != (int)me) {
+                tc_fence_after();
+                const uint32_t slot = (uint32_t)(ob * n_splits) + me;
+                const uint32_t dst = map_to_rank(sKV + slot * SLOT + (uint32_t)lane * D * 4, (uint32_t)owner);
+                constexpr int CPR = D / 4;
 #pragma unroll
-            for (int c = 0; c < D / 32; ++c) {
-                uint32_t o[32];
-                tmem_ld32(aO + c * 32, o);
-                tmem_wait_ld();
+                for (int c = 0; c < D / 32; ++c) {
+                    uint32_t o[32];
+                    tmem_ld32(aO + c * 32, o);
+                    tmem_wait_ld();
 #pragma unroll
-                for (int x = 0; x < 32; x += 4) {
-                    const int ch = (c * 8 + (x >> 2)) ^ (lane & (CPR - 1));
-                    if (n_tiles > 0)
-                        st_cluster_f4(dst + ch * 16, __uint_as_float(o[x]), __uint_as_float(o[x + 1]),
-                                      __uint_as_float(o[x + 2]), __uint_as_float(o[x + 3]));
-                    else
-                        st_cluster_f4(dst + ch * 16, 0.f, 0.f, 0.f, 0.f);  // empty split: (-inf, 0, 0)
+                    for (int x = 0; x < 32; x += 4) {
+                        const int ch = (c * 8 + (x >> 2)) ^ (lane & (CPR - 1));
+                        if (n_tiles > 0)
+                            st_cluster_f4(dst + ch * 16, __uint_as_float(o[x]), __uint_as_float(o[x + 1]),
+                                          __uint_as_float(o[x + 2]), __uint_as_float(o[x + 3]));
+                        else
+                            st_cluster_f4(dst + ch * 16, 0.f, 0.f, 0.f, 0.f);  // empty split: (-inf, 0, 0)
+                    }
                 }
+                st_cluster_f2(map_to_rank(ml_base + slot * 256 + (uint32_t)lane * 8, (uint32_t)owner), m_ref, l_sum);
             }
-            st_cluster_f2(map_to_rank(ml_base + slot * 256 + (uint32_t)lane * 8, (uint32_t)owner), m_ref, l_sum);
+            if (n_splits > 1) cluster_sync_all();                          // B2: all partial rows delivered
+            if (mine && owner == (int)me)
+                fused_finish<D>(fa, smem_raw, sKV - smem_u32(smem_raw), ob, (int)me, n_splits, lane, aO, n_tiles > 0, m_ref,
+                                l_sum, u, n_q, Hq, G, kv, (tile0 + (parity ? 0 : t)) * beams_per_tile, quarter, ch_y, ch_off);
+            tc_fence_before();
         }
-        if (n_splits > 1) cluster_sync_all();                          // B2: all partial rows delivered
-        if (mine && owner == (int)me)
-            fused_finish<D>(fa, smem_raw, sKV - smem_u32(smem_raw), ob, (int)me, n_splits, lane, aO, n_tiles > 0, m_ref,
-                            l_sum, u, n_q, Hq, G, kv, (tile0 + (parity ? 0 : t)) * beams_per_tile, quarter, ch_y, ch_off);
-        tc_fence_before();
     }
     __syncthreads();
     if (warp == 1) {
