@@ -297,7 +297,7 @@ __device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char*
     const float inv = denom > 0.f ? 1.0f / denom : 0.f;
 
     // ---- output row, 32 columns at a time ---------------------------------------------------------------------
-#pragma unroll 1
+#pragma unroll 2
     for (int c = 0; c < D / 32; ++c) {
         float acc[32];
         {
@@ -319,20 +319,27 @@ __device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char*
                 acc[x + 2] = fmaf(w, v.z, acc[x + 2]); acc[x + 3] = fmaf(w, v.w, acc[x + 3]);
             }
         }
+        // chain V rows, two levels' loads in flight at a time (each is a dependent L2 / HBM round trip)
 #pragma unroll 1
-        for (int t = 0; t < (live ? level : 0); ++t) {
-            const float e = ch_y[t];
-            const uint4* vp = reinterpret_cast<const uint4*>(fa.vs + ch_off[t]) + c * 4;
+        for (int t0 = 0; t0 < (live ? level : 0); t0 += 2) {
+            const bool two_lv = t0 + 1 < level;
+            const float e[2] = {ch_y[t0], two_lv ? ch_y[t0 + 1] : 0.f};
+            const uint4* vp0 = reinterpret_cast<const uint4*>(fa.vs + ch_off[t0]) + c * 4;
+            const uint4* vp1 = reinterpret_cast<const uint4*>(fa.vs + ch_off[two_lv ? t0 + 1 : t0]) + c * 4;
+            uint4 vv[2][4];
 #pragma unroll
-            for (int k4 = 0; k4 < 4; ++k4) {
-                const uint4 vv = __ldg(vp + k4);
-                const uint32_t va[4] = {vv.x, vv.y, vv.z, vv.w};
+            for (int k4 = 0; k4 < 4; ++k4) { vv[0][k4] = __ldg(vp0 + k4); vv[1][k4] = __ldg(vp1 + k4); }
 #pragma unroll
-                for (int e2 = 0; e2 < 4; ++e2) {
-                    acc[k4 * 8 + 2 * e2] = fmaf(e, __uint_as_float(va[e2] << 16), acc[k4 * 8 + 2 * e2]);
-                    acc[k4 * 8 + 2 * e2 + 1] = fmaf(e, __uint_as_float(va[e2] & 0xffff0000u), acc[k4 * 8 + 2 * e2 + 1]);
+            for (int lv = 0; lv < 2; ++lv)
+#pragma unroll
+                for (int k4 = 0; k4 < 4; ++k4) {
+                    const uint32_t va[4] = {vv[lv][k4].x, vv[lv][k4].y, vv[lv][k4].z, vv[lv][k4].w};
+#pragma unroll
+                    for (int e2 = 0; e2 < 4; ++e2) {
+                        acc[k4 * 8 + 2 * e2] = fmaf(e[lv], __uint_as_float(va[e2] << 16), acc[k4 * 8 + 2 * e2]);
+                        acc[k4 * 8 + 2 * e2 + 1] = fmaf(e[lv], __uint_as_float(va[e2] & 0xffff0000u), acc[k4 * 8 + 2 * e2 + 1]);
+                    }
                 }
-            }
         }
 #pragma unroll
         for (int k4 = 0; k4 < 4; ++k4) {                // 4 chunks of 8 bf16
@@ -347,14 +354,14 @@ __device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char*
         }
     }
     __syncwarp();
-    const size_t row_base = (size_t)u * n_q * Hq + kv * G;
+    // lane l knows where row l goes (-1: dead row); the copy loop fetches that by shuffle
+    const long long my_row = live ? (long long)(((size_t)u * n_q + i) * Hq + kv * G + r % G) : -1;
 #pragma unroll 4
     for (int idx = lane; idx < 32 * CPO; idx += 32) {
         const int l2 = idx / CPO, ch = idx % CPO;
-        const int r2 = quarter * 32 + l2;
-        const int i2 = beam_base + r2 / G, g2 = r2 % G;
+        const long long row = __shfl_sync(0xffffffffu, my_row, l2);
         const uint4 v = *reinterpret_cast<const uint4*>(stage + (size_t)l2 * D * 2 + ((ch ^ (l2 & (CPO - 1))) * 16));
-        if (i2 < n_q) *reinterpret_cast<uint4*>(fa.out + (row_base + (size_t)i2 * Hq + g2) * D + ch * 8) = v;
+        if (row >= 0) *reinterpret_cast<uint4*>(fa.out + (size_t)row * D + ch * 8) = v;
     }
 }
 

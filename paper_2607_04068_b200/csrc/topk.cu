@@ -203,11 +203,20 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
         const int arr = pass & 1;
         const int w = min(11, r), shift = r - w;
         const uint32_t mask = (1u << w) - 1u;
-        for (int j = tid; j < span; j += kThreads) {
-            const uint32_t idx = idx_of(j);
-            if (idx < N) {
-                const unsigned long long v = vkey(ord_at(j, idx), idx);
-                if ((v >> r) == pref) atomicAdd(&sh.hist[arr][(uint32_t)(v >> shift) & mask], 1u);
+        for (int base = 0; base < span; base += kThreads * 4) {  // 4 parked keys in flight per thread
+            uint32_t o4[4], i4[4];
+#pragma unroll
+            for (int x = 0; x < 4; ++x) {
+                const int j = base + x * kThreads + tid;
+                i4[x] = j < span ? idx_of(j) : N;
+                o4[x] = i4[x] < N ? ord_at(j, i4[x]) : 0u;
+            }
+#pragma unroll
+            for (int x = 0; x < 4; ++x) {
+                if (i4[x] < N) {
+                    const unsigned long long v = vkey(o4[x], i4[x]);
+                    if ((v >> r) == pref) atomicAdd(&sh.hist[arr][(uint32_t)(v >> shift) & mask], 1u);
+                }
             }
         }
         __syncthreads();
@@ -269,23 +278,26 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
     }
     // Now: keys with (V >> r) > pref are selected (K - rem of them); `rem` more come from the `cb` keys with
     // (V >> r) == pref, and (K - rem) + cb <= cap: gather them all, the sort decides inside the boundary bin.
-    for (int base = 0; base < span; base += kThreads) {
-        const int j = base + tid;
-        const uint32_t idx = idx_of(j);
-        bool f = false;
-        uint32_t o = 0u;
-        if (j < span && idx < N) {
-            o = ord_at(j, idx);
-            f = (vkey(o, idx) >> r) >= pref;
+    for (int base = 0; base < span; base += kThreads * 4) {
+        uint32_t o4[4], i4[4];
+#pragma unroll
+        for (int x = 0; x < 4; ++x) {
+            const int j = base + x * kThreads + tid;
+            i4[x] = j < span ? idx_of(j) : N;
+            o4[x] = i4[x] < N ? ord_at(j, i4[x]) : 0u;
         }
-        const uint32_t bal = __ballot_sync(0xffffffffu, f);
-        if (bal) {  // one shared-memory atomic per warp-iteration reserves the slots
-            const int leader = __ffs(bal) - 1;
-            uint32_t pos = 0;
-            if (lane == leader) pos = atomicAdd(&sh.cursor, (uint32_t)__popc(bal));
-            pos = __shfl_sync(0xffffffffu, pos, leader);
-            pos += __popc(bal & ((1u << lane) - 1u));
-            if (f && pos < (uint32_t)cap) sel[pos] = ((unsigned long long)(~o) << 32) | idx;
+#pragma unroll
+        for (int x = 0; x < 4; ++x) {
+            const bool f = i4[x] < N && (vkey(o4[x], i4[x]) >> r) >= pref;
+            const uint32_t bal = __ballot_sync(0xffffffffu, f);
+            if (bal) {  // one shared-memory atomic per warp-iteration reserves the slots
+                const int leader = __ffs(bal) - 1;
+                uint32_t pos = 0;
+                if (lane == leader) pos = atomicAdd(&sh.cursor, (uint32_t)__popc(bal));
+                pos = __shfl_sync(0xffffffffu, pos, leader);
+                pos += __popc(bal & ((1u << lane) - 1u));
+                if (f && pos < (uint32_t)cap) sel[pos] = ((unsigned long long)(~o4[x]) << 32) | i4[x];
+            }
         }
     }
     cluster.sync();
