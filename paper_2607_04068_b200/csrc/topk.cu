@@ -33,11 +33,17 @@
 //            passes; heavy ties simply run on into the index bits.
 //   gather   every CTA appends its qualifying keys as composites (~ord, idx) to
 //            its own list; CTA 0 pulls the lists after a cluster barrier.
+//   prune    (large slices) shared-memory atomics cost ~1 cycle per key, so
+//            before the first pass every CTA derives, from per-thread bucket
+//            maxima, a first-pass bin below which none of its keys can be
+//            selected; the first pass histograms only the keys above it and
+//            parks them in a survivor list that all later steps walk instead
+//            of the whole slice.
 //   sort     CTA 0 sorts the composites (a strict total order: the result does
-//            not depend on arrival order): bitonic, 64 keys per warp in
-//            registers with shuffles, shared memory only for the strides that
-//            cross warps; writes the first W_out as (score, parent, code),
-//            recomputing score with the same fp32 add.
+//            not depend on arrival order): rank sort up to 256; up to 1024 every
+//            warp bitonic-sorts a run of 64 in registers and the runs are merged
+//            by ranking (binary searches); writes the first W_out as (score,
+//            parent, code), recomputing score with the same fp32 add.
 // Algorithmic HBM bytes: 4 per candidate (read once) + 4 per input beam + 12
 // per selected beam.  Keys beyond the shared-memory
 // cache (paper-scale codebooks) are re-read through L2 in each pass.
@@ -60,7 +66,7 @@ constexpr int kCoarse = 64;           // coarse bins, 32 fine bins each
 constexpr int kMaxCluster = 16;       // non-portable size, used only when the device can co-schedule it
 constexpr int kSliceMin = 2048;       // do not split a user into slices smaller than this
 constexpr int kRankSortMax = 256;    // up to here a counting rank sort beats the bitonic network
-constexpr int kRegSortMax = 1024;     // register bitonic handles up to 2 keys per thread
+constexpr int kRegSortMax = 1024;     // sorted runs of 64 per warp + merge by ranking
 constexpr int kSmemBudget = 227 * 1024;
 
 struct Shared {
@@ -71,16 +77,14 @@ struct Shared {
     uint32_t sel_bin, sel_rem, sel_cnt;
     uint32_t cta_max, cta_min;     // this CTA's keys (read remotely)
     uint32_t cursor;               // length of this CTA's list (read remotely)
+    uint32_t prune_bin;            // lower bound (first-pass digit) below which no key can be selected
+    uint32_t sv_count;             // survivors of the pruning pass (may exceed the list capacity: overflow)
 };
 
 __device__ __forceinline__ uint32_t ord_of(float key) {
     uint32_t b = __float_as_uint(key);
     if (b == 0x80000000u) b = 0u;  // -0.0 == +0.0 (IEEE comparison, reading R6)
     return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
-}
-
-__device__ __forceinline__ void named_barrier(int id, int n_threads) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n_threads) : "memory");
 }
 
 // One warp: descending-bin suffix scan over 32 per-lane counts c (lane l = bin base+l).  Finds the highest
@@ -106,7 +110,7 @@ __device__ __forceinline__ void warp_select32(uint32_t c, uint32_t rem, int& bin
 __global__ void __launch_bounds__(kThreads, 1)
 topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int W_in, int C, int c_shift,
             int W_out, float* __restrict__ out_score, int32_t* __restrict__ out_parent,
-            int32_t* __restrict__ out_code, int cache_cap, int cap) {
+            int32_t* __restrict__ out_code, int cache_cap, int cap, int prune) {
     cg::cluster_group cluster = cg::this_cluster();
     const int nc = (int)cluster.num_blocks();
     const int rank = (int)cluster.block_rank();
@@ -116,7 +120,8 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Shared& sh = *reinterpret_cast<Shared*>(smem_raw);
     unsigned long long* sel = reinterpret_cast<unsigned long long*>(smem_raw + ((sizeof(Shared) + 15) / 16) * 16);
-    uint32_t* cache = reinterpret_cast<uint32_t*>(sel + cap);
+    uint2* sv = reinterpret_cast<uint2*>(sel + cap);          // survivors (ord, idx); `cap` entries iff prune
+    uint32_t* cache = reinterpret_cast<uint32_t*>(sv + (prune ? cap : 0));
 
     // ---- this rank's keys: chunks rank, rank + nc, ... of kChunk consecutive flat indices -------------
     const uint32_t N = (uint32_t)((long long)W_in * C);  // < 2^31 (validated by the API)
@@ -129,36 +134,64 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
     auto idx_of = [&](int j) -> uint32_t {
         return ((uint32_t)(j / kChunk) * (uint32_t)nc + (uint32_t)rank) * kChunk + (uint32_t)(j % kChunk);
     };
-    auto key_ord = [&](uint32_t idx) -> uint32_t {
-        const int row = c_shift >= 0 ? (int)(idx >> c_shift) : (int)(idx / (uint32_t)C);
-        const float s = sc ? __ldg(sc + row) : 0.f;
-        return ord_of(__fadd_rn(s, __ldg(lp + idx)));
-    };
-    auto ord_at = [&](int j, uint32_t idx) -> uint32_t { return j < cache_cap ? cache[j] : key_ord(idx); };
 
     for (int b = tid; b < 2 * kBins + 2 * kCoarse; b += kThreads) (&sh.hist[0][0])[b] = 0;  // hist + coarse
-    if (tid == 0) sh.cursor = 0;
+    if (tid == 0) { sh.cursor = 0; sh.prune_bin = 0; sh.sv_count = 0; }
 
     // ---- load: the one pass over HBM ---------------------------------------------------
+    // All loads of an iteration are issued before any is consumed: indices are clamped instead of branched
+    // around (a branch per key made ptxas wait for each load pair in turn: 8 round trips instead of 1).
+    // bm[]: running maxima of 4 disjoint key subsets per thread ("buckets"), used to prune the histograms.
     uint32_t mx = 0u, mn = 0xffffffffu;
-    for (int base = 0; base < span; base += kThreads * kUnroll) {
-        // all 2 * kUnroll loads are issued before any is consumed: indices are clamped instead of branched
-        // around (a branch per key made ptxas wait for each load pair in turn: 8 round trips instead of 1)
-        float lv[kUnroll], sv[kUnroll];
+    uint32_t bm[4] = {0u, 0u, 0u, 0u};
+    const bool vec = (N & 3u) == 0 && (!sc || (C & 3) == 0) && ((reinterpret_cast<uintptr_t>(lp) & 15u) == 0) &&
+                     (cache_cap & 3) == 0;
+    if (vec) {
+        // 16-byte loads: 4 consecutive candidates of one parent beam per load, 64 KB in flight per CTA
+        const int span4 = span >> 2;
+        for (int base4 = 0; base4 < span4; base4 += kThreads * kUnroll) {
+            float4 lv[kUnroll];
+            float sv[kUnroll];
 #pragma unroll
-        for (int x = 0; x < kUnroll; ++x) {
-            const uint32_t idx = min(idx_of(base + x * kThreads + tid), N - 1);
-            const int row = c_shift >= 0 ? (int)(idx >> c_shift) : (int)(idx / (uint32_t)C);
-            lv[x] = __ldg(lp + idx);
-            sv[x] = sc ? __ldg(sc + row) : 0.f;
+            for (int x = 0; x < kUnroll; ++x) {
+                const uint32_t idx = min(idx_of(4 * (base4 + x * kThreads + tid)), N - 4);
+                const int row = c_shift >= 0 ? (int)(idx >> c_shift) : (int)(idx / (uint32_t)C);
+                lv[x] = __ldg(reinterpret_cast<const float4*>(lp + idx));
+                sv[x] = sc ? __ldg(sc + row) : 0.f;
+            }
+#pragma unroll
+            for (int x = 0; x < kUnroll; ++x) {
+                const int j = 4 * (base4 + x * kThreads + tid);
+                if (j < span && idx_of(j) < N) {
+                    uint4 o;
+                    o.x = ord_of(__fadd_rn(sv[x], lv[x].x)); o.y = ord_of(__fadd_rn(sv[x], lv[x].y));
+                    o.z = ord_of(__fadd_rn(sv[x], lv[x].z)); o.w = ord_of(__fadd_rn(sv[x], lv[x].w));
+                    if (j < cache_cap) *reinterpret_cast<uint4*>(cache + j) = o;
+                    const uint32_t hi = max(max(o.x, o.y), max(o.z, o.w)), lo4 = min(min(o.x, o.y), min(o.z, o.w));
+                    mx = max(mx, hi); mn = min(mn, lo4);
+                    bm[x & 3] = max(bm[x & 3], hi);
+                }
+            }
         }
+    } else {
+        for (int base = 0; base < span; base += kThreads * kUnroll) {
+            float lv[kUnroll], sv[kUnroll];
 #pragma unroll
-        for (int x = 0; x < kUnroll; ++x) {
-            const int j = base + x * kThreads + tid;
-            if (j < span && idx_of(j) < N) {
-                const uint32_t o = ord_of(__fadd_rn(sv[x], lv[x]));
-                if (j < cache_cap) cache[j] = o;
-                mx = max(mx, o); mn = min(mn, o);
+            for (int x = 0; x < kUnroll; ++x) {
+                const uint32_t idx = min(idx_of(base + x * kThreads + tid), N - 1);
+                const int row = c_shift >= 0 ? (int)(idx >> c_shift) : (int)(idx / (uint32_t)C);
+                lv[x] = __ldg(lp + idx);
+                sv[x] = sc ? __ldg(sc + row) : 0.f;
+            }
+#pragma unroll
+            for (int x = 0; x < kUnroll; ++x) {
+                const int j = base + x * kThreads + tid;
+                if (j < span && idx_of(j) < N) {
+                    const uint32_t o = ord_of(__fadd_rn(sv[x], lv[x]));
+                    if (j < cache_cap) cache[j] = o;
+                    mx = max(mx, o); mn = min(mn, o);
+                    bm[x & 3] = max(bm[x & 3], o);
+                }
             }
         }
     }
@@ -192,34 +225,153 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
         return ((unsigned long long)(o & lowmask) << nbi) | (unsigned long long)(~idx & idxmask);
     };
 
+    // Walk ALL keys of this rank, warp-uniformly: fn(valid, ord, idx).  Parked keys come from shared memory,
+    // 4 in flight per thread; keys beyond the cache are recomputed from global memory (L2) with the same
+    // batched, branch-free loads as the first pass.
+    auto scan_all = [&](auto&& fn) {
+        const int n_c = min(span, cache_cap);
+        for (int base = 0; base < n_c; base += kThreads * 4) {
+            uint32_t o4[4], i4[4];
+#pragma unroll
+            for (int x = 0; x < 4; ++x) {
+                const int j = base + x * kThreads + tid;
+                i4[x] = j < n_c ? idx_of(j) : N;
+                o4[x] = i4[x] < N ? cache[j] : 0u;
+            }
+#pragma unroll
+            for (int x = 0; x < 4; ++x) fn(i4[x] < N, o4[x], i4[x]);
+        }
+        if (span <= cache_cap) return;
+        if (vec) {
+            for (int base4 = cache_cap >> 2; base4 < (span >> 2); base4 += kThreads * 4) {
+                float4 lv[4];
+                float sv[4];
+                uint32_t ib[4];
+#pragma unroll
+                for (int x = 0; x < 4; ++x) {
+                    const int j = 4 * (base4 + x * kThreads + tid);
+                    const uint32_t id = j < span ? idx_of(j) : N;
+                    ib[x] = id;
+                    const uint32_t idc = min(id, N - 4);
+                    const int row = c_shift >= 0 ? (int)(idc >> c_shift) : (int)(idc / (uint32_t)C);
+                    lv[x] = __ldg(reinterpret_cast<const float4*>(lp + idc));
+                    sv[x] = sc ? __ldg(sc + row) : 0.f;
+                }
+#pragma unroll
+                for (int x = 0; x < 4; ++x) {
+                    const bool ok = ib[x] < N;
+                    fn(ok, ord_of(__fadd_rn(sv[x], lv[x].x)), ib[x]);
+                    fn(ok, ord_of(__fadd_rn(sv[x], lv[x].y)), ib[x] + 1);
+                    fn(ok, ord_of(__fadd_rn(sv[x], lv[x].z)), ib[x] + 2);
+                    fn(ok, ord_of(__fadd_rn(sv[x], lv[x].w)), ib[x] + 3);
+                }
+            }
+        } else {
+            for (int base = cache_cap; base < span; base += kThreads * 4) {
+                float lv[4], sv[4];
+                uint32_t ib[4];
+#pragma unroll
+                for (int x = 0; x < 4; ++x) {
+                    const int j = base + x * kThreads + tid;
+                    const uint32_t id = j < span ? idx_of(j) : N;
+                    ib[x] = id;
+                    const uint32_t idc = min(id, N - 1);
+                    const int row = c_shift >= 0 ? (int)(idc >> c_shift) : (int)(idc / (uint32_t)C);
+                    lv[x] = __ldg(lp + idc);
+                    sv[x] = sc ? __ldg(sc + row) : 0.f;
+                }
+#pragma unroll
+                for (int x = 0; x < 4; ++x) fn(ib[x] < N, ord_of(__fadd_rn(sv[x], lv[x])), ib[x]);
+            }
+        }
+    };
+
     // ---- radix select on V over the parked keys ----------------------------------------------------
     const uint32_t K = (uint32_t)W_out;
     uint32_t rem = K;                 // keys still to take from the candidate set
     unsigned long long pref = 0ull;   // value of V >> r shared by every candidate
     int r = nb + nbi;                 // unresolved low bits of V (<= 63)
     uint32_t cb = N;                  // candidates (= keys with V >> r == pref)
+
+    // ---- pruning bound (large slices): shared-memory atomics cost ~1 cycle per key, so a histogram over
+    // all keys would dominate.  Each thread kept the maxima of 4 disjoint subsets of its keys; if K of this
+    // CTA's 2048 bucket maxima lie in first-pass bins >= b, at least K real keys do, so the W_out-th key of
+    // the whole user cannot lie below bin b.  Every CTA may drop its keys below its own b: the cluster-wide
+    // boundary bin found from the pruned histograms is >= every CTA's b, and exact from there upwards.
+    bool pruning = prune && N > (uint32_t)cap && r > 0;
+    if (pruning) {
+        const int w0 = min(11, r), shift0 = r - w0;
+#pragma unroll
+        for (int b = 0; b < 4; ++b)
+            if (bm[b]) atomicAdd(&sh.hist[1][(uint32_t)((((unsigned long long)(bm[b] & lowmask)) << nbi) >> shift0)], 1u);
+        __syncthreads();
+        {
+            const uint4 v = reinterpret_cast<const uint4*>(&sh.hist[1][0])[tid];
+            uint32_t c4 = v.x + v.y + v.z + v.w;
+            c4 += __shfl_xor_sync(0xffffffffu, c4, 1);
+            c4 += __shfl_xor_sync(0xffffffffu, c4, 2);
+            c4 += __shfl_xor_sync(0xffffffffu, c4, 4);
+            if ((lane & 7) == 0) sh.coarse[1][tid >> 3] = c4;
+        }
+        __syncthreads();
+        if (warp == 0) {
+            const uint32_t chi = sh.coarse[1][32 + lane], clo = sh.coarse[1][lane];
+            const uint32_t tot_hi = __reduce_add_sync(0xffffffffu, chi), tot_lo = __reduce_add_sync(0xffffffffu, clo);
+            if (tot_hi + tot_lo >= K) {             // (fewer buckets than K: no bound)
+                const bool in_hi = K <= tot_hi;
+                int cbin, fbin; uint32_t rem2, rem3, cnt;
+                warp_select32(in_hi ? chi : clo, in_hi ? K : K - tot_hi, cbin, rem2, cnt);
+                const int coarse_bin = (in_hi ? 32 : 0) + cbin;
+                warp_select32(sh.hist[1][coarse_bin * 32 + lane], rem2, fbin, rem3, cnt);
+                if (lane == 0) sh.prune_bin = (uint32_t)(coarse_bin * 32 + fbin);
+            }
+        }
+        __syncthreads();                             // hist[1] / coarse[1] are re-zeroed during pass 0
+    }
+    const uint32_t prune_bin = sh.prune_bin;
+    bool use_sv = false;                             // later loops walk the survivor list instead of all keys
+    uint32_t n_sv = 0;
 #pragma unroll 1
     for (int pass = 0; (K - rem) + cb > (uint32_t)cap; ++pass) {  // same decision in every CTA
         const int arr = pass & 1;
         const int w = min(11, r), shift = r - w;
         const uint32_t mask = (1u << w) - 1u;
-        for (int base = 0; base < span; base += kThreads * 4) {  // 4 parked keys in flight per thread
-            uint32_t o4[4], i4[4];
-#pragma unroll
-            for (int x = 0; x < 4; ++x) {
-                const int j = base + x * kThreads + tid;
-                i4[x] = j < span ? idx_of(j) : N;
-                o4[x] = i4[x] < N ? ord_at(j, i4[x]) : 0u;
+        if (use_sv) {
+            for (uint32_t e = tid; e < n_sv; e += kThreads) {
+                const uint2 k = sv[e];
+                const unsigned long long v = vkey(k.x, k.y);
+                if ((v >> r) == pref) atomicAdd(&sh.hist[arr][(uint32_t)(v >> shift) & mask], 1u);
             }
-#pragma unroll
-            for (int x = 0; x < 4; ++x) {
-                if (i4[x] < N) {
-                    const unsigned long long v = vkey(o4[x], i4[x]);
+        } else {
+            if (pruning && pass == 0) {
+                // first pass of a pruned run: nearly every key fails the bound, so the test must be cheap.
+                // While the digit lies wholly inside the ord bits (shift >= nbi) it is a 32-bit shift.
+                const bool narrow = shift >= nbi;
+                const int sh32 = narrow ? shift - nbi : 0;
+                scan_all([&](bool ok, uint32_t o, uint32_t idx) {
+                    if (!ok) return;
+                    uint32_t dg;
+                    if (narrow) dg = (o & lowmask) >> sh32;
+                    else dg = (uint32_t)(vkey(o, idx) >> shift) & mask;
+                    if (dg >= prune_bin) {                   // rare: K-ish keys per user
+                        atomicAdd(&sh.hist[arr][dg], 1u);
+                        const uint32_t pos = atomicAdd(&sh.sv_count, 1u);
+                        if (pos < (uint32_t)cap) sv[pos] = make_uint2(o, idx);
+                    }
+                });
+            } else {
+                scan_all([&](bool ok, uint32_t o, uint32_t idx) {
+                    if (!ok) return;
+                    const unsigned long long v = vkey(o, idx);
                     if ((v >> r) == pref) atomicAdd(&sh.hist[arr][(uint32_t)(v >> shift) & mask], 1u);
-                }
+                });
             }
         }
         __syncthreads();
+        if (pruning && pass == 0) {                      // list complete?  else fall back to scanning all keys
+            n_sv = sh.sv_count;
+            use_sv = n_sv <= (uint32_t)cap;
+        }
         {   // coarse histogram: 32 fine bins = 8 threads x 4 bins
             const uint4 v = reinterpret_cast<const uint4*>(&sh.hist[arr][0])[tid];
             uint32_t s = v.x + v.y + v.z + v.w;
@@ -278,27 +430,25 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
     }
     // Now: keys with (V >> r) > pref are selected (K - rem of them); `rem` more come from the `cb` keys with
     // (V >> r) == pref, and (K - rem) + cb <= cap: gather them all, the sort decides inside the boundary bin.
-    for (int base = 0; base < span; base += kThreads * 4) {
-        uint32_t o4[4], i4[4];
-#pragma unroll
-        for (int x = 0; x < 4; ++x) {
-            const int j = base + x * kThreads + tid;
-            i4[x] = j < span ? idx_of(j) : N;
-            o4[x] = i4[x] < N ? ord_at(j, i4[x]) : 0u;
+    auto take = [&](bool ok, uint32_t o, uint32_t idx) {
+        const bool f = ok && (vkey(o, idx) >> r) >= pref;
+        const uint32_t bal = __ballot_sync(0xffffffffu, f);
+        if (bal) {  // one shared-memory atomic per warp-iteration reserves the slots
+            const int leader = __ffs(bal) - 1;
+            uint32_t pos = 0;
+            if (lane == leader) pos = atomicAdd(&sh.cursor, (uint32_t)__popc(bal));
+            pos = __shfl_sync(0xffffffffu, pos, leader) + __popc(bal & ((1u << lane) - 1u));
+            if (f && pos < (uint32_t)cap) sel[pos] = ((unsigned long long)(~o) << 32) | idx;
         }
-#pragma unroll
-        for (int x = 0; x < 4; ++x) {
-            const bool f = i4[x] < N && (vkey(o4[x], i4[x]) >> r) >= pref;
-            const uint32_t bal = __ballot_sync(0xffffffffu, f);
-            if (bal) {  // one shared-memory atomic per warp-iteration reserves the slots
-                const int leader = __ffs(bal) - 1;
-                uint32_t pos = 0;
-                if (lane == leader) pos = atomicAdd(&sh.cursor, (uint32_t)__popc(bal));
-                pos = __shfl_sync(0xffffffffu, pos, leader);
-                pos += __popc(bal & ((1u << lane) - 1u));
-                if (f && pos < (uint32_t)cap) sel[pos] = ((unsigned long long)(~o4[x]) << 32) | i4[x];
-            }
+    };
+    if (use_sv) {
+        for (uint32_t base = 0; base < n_sv; base += kThreads) {
+            const uint32_t e = base + tid;
+            const uint2 k = e < n_sv ? sv[e] : make_uint2(0u, N);
+            take(e < n_sv, k.x, k.y);
         }
+    } else {
+        scan_all(take);
     }
     cluster.sync();
 
@@ -336,31 +486,26 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
         __syncthreads();
         if (tid < n_g) sel[rank_of] = mine;
         __syncthreads();
-    } else if (S <= kRegSortMax) {
-        // registers: warp w owns elements [64w, 64w+64): lane holds e0 = 64w + lane and e1 = e0 + 32.
-        // Strides < 32 exchange by shuffle, stride 32 is thread-local, strides >= 64 go through shared memory.
-        const int n_warps = S >> 6, n_thr = n_warps * 32;
-        if (warp < n_warps) {
-            const int e0 = warp * 64 + lane, e1 = e0 + 32;
-            unsigned long long a = sel[e0], b = sel[e1];
-            for (int k = 2; k <= S; k <<= 1) {
+    } else if (S <= kRegSortMax && cache_cap >= 2 * S) {
+        // (1) every warp bitonic-sorts a run of 64 composites in registers: lane holds e0 = 64w + lane and
+        //     e1 = e0 + 32; stride 32 is thread-local, smaller strides exchange by shuffle; no barrier.
+        // (2) merge by ranking: final position = position in the own run + lower bounds in the other runs
+        //     (binary searches over shared memory); the result goes to the dead key cache.
+        const int n_runs = S >> 6;
+        const int e0 = warp * 64 + lane, e1 = e0 + 32;
+        unsigned long long a = ~0ull, b = ~0ull;
+        if (warp < n_runs) {
+            a = sel[e0]; b = sel[e1];
+            for (int k = 2; k <= 64; k <<= 1) {
                 for (int j = k >> 1; j > 0; j >>= 1) {
-                    if (j >= 64) {
-                        sel[e0] = a; sel[e1] = b;
-                        named_barrier(1, n_thr);
-                        const unsigned long long pa = sel[e0 ^ j], pb = sel[e1 ^ j];
-                        const bool keep_min = ((e0 & j) == 0) == ((e0 & k) == 0);  // same for e1: j, k >= 64
-                        a = keep_min ? min(a, pa) : max(a, pa);
-                        b = keep_min ? min(b, pb) : max(b, pb);
-                        named_barrier(1, n_thr);
-                    } else if (j == 32) {
-                        const bool up = (e0 & k) == 0;
-                        if ((a > b) == up) { const unsigned long long t = a; a = b; b = t; }
+                    if (j == 32) {
+                        if (a > b) { const unsigned long long t = a; a = b; b = t; }  // k = 64: ascending
                     } else {
                         const unsigned long long pa = __shfl_xor_sync(0xffffffffu, a, j);
                         const unsigned long long pb = __shfl_xor_sync(0xffffffffu, b, j);
                         const bool lower = (lane & j) == 0;
-                        const bool min_a = lower == ((e0 & k) == 0), min_b = lower == ((e1 & k) == 0);
+                        // directions from the position INSIDE the run (lane, lane + 32): every run ascending
+                        const bool min_a = lower == ((lane & k) == 0), min_b = lower == (((lane + 32) & k) == 0);
                         a = min_a ? min(a, pa) : max(a, pa);
                         b = min_b ? min(b, pb) : max(b, pb);
                     }
@@ -368,6 +513,27 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
             }
             sel[e0] = a; sel[e1] = b;
         }
+        __syncthreads();
+        unsigned long long* dst = reinterpret_cast<unsigned long long*>(cache);
+        if (warp < n_runs) {
+            int ra = 0, rb = 0;                          // (the own run contributes the position inside it)
+#pragma unroll 4
+            for (int w2 = 0; w2 < n_runs; ++w2) {        // independent binary searches: unrolled for overlap
+                const unsigned long long* run = sel + w2 * 64;
+                int ca = 0, cb2 = 0;
+#pragma unroll
+                for (int st = 32; st > 0; st >>= 1) {
+                    if (run[ca + st - 1] < a) ca += st;
+                    if (run[cb2 + st - 1] < b) cb2 += st;
+                }
+                if (ca == 63 && run[63] < a) ca = 64;
+                if (cb2 == 63 && run[63] < b) cb2 = 64;
+                ra += ca; rb += cb2;
+            }
+            dst[ra] = a; dst[rb] = b;                    // composites are distinct: a permutation
+        }
+        __syncthreads();
+        for (int i2 = tid; i2 < S; i2 += kThreads) sel[i2] = dst[i2];
         __syncthreads();
     } else {
         for (int k = 2; k <= S; k <<= 1) {
@@ -384,11 +550,11 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
         }
     }
     for (int rr = tid; rr < (int)K; rr += kThreads) {
-        const uint32_t idx = (uint32_t)sel[rr];
+        const uint32_t idx = min((uint32_t)sel[rr], N - 1);  // (clamp: memory safety on NaN-poisoned input)
         const int row = c_shift >= 0 ? (int)(idx >> c_shift) : (int)(idx / (uint32_t)C);
         const int code = (int)idx - row * C;
         const float s = sc ? __ldg(sc + row) : 0.f;
-        out_score[(size_t)u * W_out + rr] = __fadd_rn(s, __ldg(lp + min(idx, N - 1)));
+        out_score[(size_t)u * W_out + rr] = __fadd_rn(s, __ldg(lp + idx));
         out_parent[(size_t)u * W_out + rr] = row;
         out_code[(size_t)u * W_out + rr] = code;
     }
@@ -405,7 +571,9 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
                 cudaStream_t st) {
     const long long N = (long long)W_in * C;
     const int cap = next_pow2(W_out) * 2 < 128 ? 128 : next_pow2(W_out) * 2;  // sort buffer entries
-    const size_t fixed = ((sizeof(Shared) + 15) / 16) * 16 + (size_t)cap * 8;
+    // pruning pays once a thread holds many keys (>= 16: slices of 8192) and needs K <= the 2048 buckets of a CTA
+    const int prune = (N / kMaxCluster >= 8192 || N >= 32768) && W_out <= 2048 ? 1 : 0;
+    const size_t fixed = ((sizeof(Shared) + 15) / 16) * 16 + (size_t)cap * 8 * (prune ? 2 : 1);
     const long long cache_max = ((long long)kSmemBudget - (long long)fixed) / 4;
     static bool attr_done = false;  // idempotent; a benign race at worst repeats the calls
     if (!attr_done) {
@@ -426,7 +594,7 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
     int nc = 1, cache_cap = 0;
     auto configure = [&](int n) {
         const long long slice = ((N + kChunk - 1) / kChunk + n - 1) / n * kChunk;  // whole chunks
-        cache_cap = (int)(slice < cache_max ? slice : cache_max);
+        cache_cap = (int)(slice < cache_max ? slice : cache_max) & ~3;  // whole 16-byte groups
         cfg.gridDim = dim3((unsigned)(B * n));
         cfg.dynamicSmemBytes = fixed + (size_t)cache_cap * 4;
         at[0].val.clusterDim.x = n;
@@ -452,7 +620,7 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
     int c_shift = -1;
     if ((C & (C - 1)) == 0) { c_shift = 0; while ((1 << c_shift) < C) ++c_shift; }
     STARK_CUDA_TRY(cudaLaunchKernelEx(&cfg, topk_kernel, logp, score, W_in, C, c_shift, W_out, out_score,
-                                      out_parent, out_code, cache_cap, cap));
+                                      out_parent, out_code, cache_cap, cap, prune));
     return STARK_OK;
 }
 
