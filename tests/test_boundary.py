@@ -64,6 +64,14 @@ def test_validation_before_cuda(L):
     assert L.stark_beam_topk(p, None, 1, 1 << 16, 1 << 16, 4, p, p, p, None, 0, None) == -1        # >= 2^31
     assert L.stark_kv_append_reorg(ctypes.byref(sh), 0, 1, p, p, p, p, p, p, None) == -1           # level < 1
     assert L.stark_kv_append_reorg(ctypes.byref(sh), 2, 1, p, p, None, p, p, p, None) == -1        # parent missing
+    # fused decode attention: argument errors first, then "bf16 only" (fp32 shapes compose A1 + A2)
+    bf = sb.make_shape(2, 8, 2, 128, 3, 8, torch.bfloat16)
+    assert L.stark_decode_attn(ctypes.byref(bf), None, 1, 0, p, p, p, 4, 4, p, p, p, p, None) == -1   # q missing
+    assert L.stark_decode_attn(ctypes.byref(bf), p, 1, 4, p, p, p, 4, 4, p, p, p, p, None) == -1      # level > d
+    assert L.stark_decode_attn(ctypes.byref(bf), p, 9, 1, p, p, p, 4, 4, p, p, p, p, None) == -1      # n_q > Wmax
+    assert L.stark_decode_attn(ctypes.byref(bf), p, 1, 1, p, p, p, 4, 4, p, p, None, p, None) == -1   # anc missing
+    assert L.stark_decode_attn(ctypes.byref(sh), p, 1, 0, p, p, p, 4, 4, p, p, p, p, None) == -2      # fp32
+    assert L.stark_calib_stream_read(None, 64, p, None) == -1
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="only meaningful without a GPU")
