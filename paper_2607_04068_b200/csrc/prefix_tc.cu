@@ -1,4 +1,5 @@
-// A1 (tensor-core form): stark_prefix_attn for bf16, any number of query rows.
+// A1 and A1+A2 (tensor-core form): stark_prefix_attn and the fused stark_decode_attn for bf16, any number
+// of query rows.
 //
 // the conventional path recomputes attention over the shared
 // user-history prefix once per beam; STARK computes it once.  Here all
@@ -6,34 +7,44 @@
 // dimension of a dense contraction against that user's prefix K/V tiles, so
 // each prefix byte is fetched once per step per CTA instead of once per beam.
 // This is a real GEMM-shaped op (AI ~ M flop per KV byte), so it runs on the
-// 5th-generation tensor cores, organised like a two-tile flash-attention
-// forward whose epilogue emits split-softmax partials:
+// 5th-generation tensor cores, organised like a two-accumulator flash-attention
+// forward:
 //
-//   * one CTA per (pair of 128-row Q tiles, KV head, prefix split, user): 256
-//     query rows share every K/V tile staged in shared memory;
+//   * 384 threads = 3 warpgroups: warpgroup 0 holds the TMA producer warp and
+//     the MMA issuer warp (one elected lane each; two idle warps), warpgroups 1
+//     and 2 are the softmax warpgroups of accumulator sets 0 and 1, one TMEM
+//     lane (= query row) per thread.  setmaxnreg moves registers from
+//     warpgroup 0 to the softmax warpgroups, whose threads keep a whole S row
+//     (128 fp32) in registers between its maximum and its exponentials;
 //   * Q tiles and K/V tiles arrive by TMA (cp.async.bulk.tensor, 128-byte
-//     swizzle); K and V alternate through one NS-slot mbarrier ring;
-//   * S_t = Q_t K^T by tcgen05.mma (SS, both operands K-major) into TMEM, one
-//     128-column accumulator per Q tile; P_t (bf16) overwrites S_t in place;
+//     swizzle); K and V alternate through one NS-slot mbarrier ring; the first
+//     loads are issued before TMEM is allocated;
+//   * S_t = Q K^T by tcgen05.mma (SS, both operands K-major) into TMEM, one
+//     128-column accumulator per set; P_t (bf16) overwrites S_t in place;
 //     O_t += P_t V by tcgen05.mma with A = P_t from TMEM and B = V from shared
 //     memory (MN-major descriptor: V is [kv][D] with D contiguous);
 //     TMEM columns: S0/P0 [0,128) S1/P1 [128,256) O0 [256,256+D) O1 [384,384+D);
-//   * two softmax warpgroups, one per Q tile, one TMEM lane (= query row) per
-//     thread.  The MMA warp issues  PV0_j, QK0_{j+1}, PV1_j, QK1_{j+1}, ...  so the
-//     tensor pipe works on one tile while the other tile's warpgroup runs its
-//     softmax (exp2 on the MUFU pipe) -- the two units stay busy together;
-//   * softmax streams its S row from TMEM twice (max, then exp2 + pack), 32
-//     columns at a time, so it needs few registers; running reference maximum
-//     with lazy rescale (O is touched only when a row maximum grows by > 2^8);
-//     the tensor pipe executes in issue order, so when S_t(j) is ready PV_t(j-1)
-//     has completed and O_t may be rescaled without another barrier;
-//   * epilogue: tcgen05.ld the O rows and emit the split-softmax partials
-//     (m, l, o) that stark_tree_attn_step merges by log-sum-exp.
+//   * the MMA warp issues  PV_0, QK_0(next), PV_1, QK_1(next), ...  so the tensor
+//     pipe works for one set while the other set's warpgroup runs its softmax
+//     (exp2 on the MUFU pipe).  The pipe executes in issue order, so when
+//     S_t(j) is ready PV_t(j-1) has completed and O_t may be rescaled (lazily:
+//     only when a row maximum grows by > 2^8) without another barrier;
+//   * pair mode: the CTA owns two 128-row Q tiles, set t = Q tile t, every K/V
+//     tile serves 256 rows.  Parity mode (when its doubled CTA count still
+//     fits one wave): the CTA owns one Q tile, set t = the KV tiles of parity
+//     t; the two partial softmaxes are folded inside the CTA at the end;
+//   * FUSED = false: the epilogue stages the O rows in the idle K/V ring and
+//     writes coalesced split-softmax partials (m, l, o) for
+//     stark_tree_attn_step.  FUSED = true: the prefix splits of one (Q tiles,
+//     KV head, user) are a thread-block cluster; partial rows are exchanged
+//     through distributed shared memory and the owner of each 32-row block
+//     merges them, adds the suffix chain (scores computed while the first
+//     tiles are in flight), normalises and writes bf16 rows -- no partial ever
+//     reaches HBM.
 //
 // Decode step 0 (a single query per user, M = G rows) runs through the same
-// kernel: the contraction is then a pure HBM stream of the prefix (the tensor
-// pipe needs ~1/3 of the tile's HBM time), and warps without live rows skip
-// their softmax.
+// kernel: the contraction is then a pure HBM stream of the prefix, and warps
+// without live rows skip their softmax.
 // Every mbarrier wait is bounded (trap after ~1 s) so that a protocol bug
 // surfaces as a launch failure instead of a hung GPU.
 #include <cuda.h>
