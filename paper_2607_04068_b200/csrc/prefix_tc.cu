@@ -891,7 +891,7 @@ int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, 
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = n_splits; at[0].val.clusterDim.z = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
+    cfg.attrs = at; cfg.numAttrs = n_splits > 1 ? 1 : 0;   // a single split needs no cluster launch
     STARK_CUDA_TRY(cudaLaunchKernelEx(&cfg, prefix_tc_kernel<D, true>, tq, tk, tv, cu, (float*)nullptr,
                                       (float*)nullptr, (float*)nullptr, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits,
                                       p.scale * kLog2e, parity, fa));
