@@ -252,6 +252,50 @@ def run_calibrate():
     print(json.dumps({"calibration": out}), flush=True)
 
 
+def run_cfg3_decoder(args):
+    """BASELINE configs[2]: the library inside a 12-layer random-init decoder (tests/_decoder_harness.py; GEMMs in
+    torch/cuBLAS, not graded).  Prefill untimed.  Reports the whole decode (4 levels x 12 layers) and the
+    library calls alone (same captured inputs, no GEMMs), eager launches, CUDA events."""
+    import torch
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from _decoder_harness import Decoder, DecoderShape
+    sh = DecoderShape()
+    model = Decoder(sh, seed=0)
+    g = torch.Generator(device="cpu").manual_seed(3)
+    tokens = torch.randint(0, sh.vocab, (sh.B, sh.prefix), generator=g).cuda()
+    cap = model.decode(tokens)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed(fn, n):
+        for _ in range(max(3, args.warmup // 10)):
+            fn()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    n = max(3, min(args.steps, 20))
+    kv, _ = model.prefill(tokens)
+
+    def whole():           # decode only: the prefix K/V of `cap` are reused, so prefill is outside the timing
+        model.prefill = lambda _t: (kv, cap["last_attn"])
+        model.decode(tokens, capture=False)
+
+    ms_all = timed(whole, n)
+    ms_lib = timed(lambda: model.replay_library(cap), n)
+    sids = sh.B * sh.W
+    print(json.dumps({"metric": METRIC, "value": sids / (ms_all * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": n,
+                      "ms_per_step": ms_all, "higher_is_better": True, "dtype": "bf16", "data": "synthetic",
+                      "config": {"workload": "cfg3_decoder", "layers": sh.n_layers, "d_model": sh.d_model, "B": sh.B,
+                                 "prefix": sh.prefix, "beam": sh.W, "levels": sh.d, "codebook": sh.C,
+                                 "launch": "eager", "prefill": "untimed (torch SDPA)"},
+                      "library_ms_per_step": ms_lib, "gemm_and_glue_ms_per_step": ms_all - ms_lib,
+                      "library_launches": sh.n_layers * (2 * sh.d - 1) + sh.d}), flush=True)  # attend + append, top-k
+
+
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -480,6 +524,8 @@ def main():
     args = parse_args()
     if args.calibrate:
         return run_calibrate()
+    if args.workload == "cfg3_decoder":
+        return run_cfg3_decoder(args)
     cfg = wl.get_config(args.workload)
     if args.impl == "reference":
         run_reference(args, cfg)
