@@ -81,14 +81,19 @@ class Decoder:
             x = self._ffn(lw, x + o.reshape(B, L, -1) @ lw["out"])
         return kv, last_attn
 
-    def decode(self, tokens: torch.Tensor, capture: bool = True) -> Dict[str, list]:
+    def decode(self, tokens: torch.Tensor, capture: bool = True, state=None) -> Dict[str, list]:
         """Semantic-ID beam search over d levels through the library.  Returns the selections per level and, if
-        `capture`, every layer's (q, k_new, v_new, attention out) per step plus the fp32 log-probs."""
+        `capture`, every layer's (q, k_new, v_new, attention out) per step plus the fp32 log-probs.
+        `state` = (prefix K/V per layer, last-position attention, StarkLayer list) of an earlier call: skips the
+        prefill and every allocation of library buffers, so that the decode loop is CUDA-graph capturable."""
         sh = self.sh
         B, L = tokens.shape
-        kv, last_attn = self.prefill(tokens)
-        cu = (torch.arange(B + 1, device=self.dev, dtype=torch.int32) * L).contiguous()
-        layers = [StarkLayer(B, sh.Hq, sh.Hkv, sh.D, sh.d, sh.W, torch.bfloat16, k, v, cu, L) for k, v in kv]
+        if state is None:
+            kv, last_attn = self.prefill(tokens)
+            cu = (torch.arange(B + 1, device=self.dev, dtype=torch.int32) * L).contiguous()
+            layers = [StarkLayer(B, sh.Hq, sh.Hkv, sh.D, sh.d, sh.W, torch.bfloat16, k, v, cu, L) for k, v in kv]
+        else:
+            kv, last_attn, layers = state
         cap = dict(q=[], k=[], v=[], out=[], logp=[], sel=[], prefix_kv=kv, last_attn=last_attn)
         widths, w_in = [], 1
         for t in range(sh.d):
