@@ -34,19 +34,24 @@
 //   gather   every CTA appends its qualifying keys as composites (~ord, idx) to
 //            its own list; CTA 0 pulls the lists after a cluster barrier.
 //   prune    (large slices) shared-memory atomics cost ~1 cycle per key, so
-//            before the first pass every CTA derives, from per-thread bucket
-//            maxima, a first-pass bin below which none of its keys can be
-//            selected; the first pass histograms only the keys above it and
-//            parks them in a survivor list that all later steps walk instead
-//            of the whole slice.
+//            every CTA first derives a bound L such that at least W_out of its
+//            own keys are >= L (the W_out-th largest of its per-thread bucket
+//            maxima): no key below L can be selected.  The first pass touches
+//            the histogram only for keys >= L and parks them in a survivor list
+//            that all later steps walk instead of the whole slice.  Keys beyond
+//            the shared-memory cache are never parked: they are streamed ONCE
+//            against L, and whenever the survivor list fills up L is
+//            re-tightened from the list itself and the list compacted (a
+//            streaming top-K).  Bursts or heavy ties that overflow the list fall
+//            back to re-reading those keys through L2.
 //   sort     CTA 0 sorts the composites (a strict total order: the result does
 //            not depend on arrival order): rank sort up to 256; up to 1024 every
 //            warp bitonic-sorts a run of 64 in registers and the runs are merged
 //            by ranking (binary searches); writes the first W_out as (score,
 //            parent, code), recomputing score with the same fp32 add.
 // Algorithmic HBM bytes: 4 per candidate (read once) + 4 per input beam + 12
-// per selected beam.  Keys beyond the shared-memory
-// cache (paper-scale codebooks) are re-read through L2 in each pass.
+// per selected beam; keys beyond the shared-memory
+// cache (paper-scale codebooks) are read once (see `prune`).
 #include <cooperative_groups.h>
 
 #include "common.cuh"
@@ -77,7 +82,9 @@ struct Shared {
     uint32_t sel_bin, sel_rem, sel_cnt;
     uint32_t cta_max, cta_min;     // this CTA's keys (read remotely)
     uint32_t cursor;               // length of this CTA's list (read remotely)
-    uint32_t prune_bin;            // lower bound (first-pass digit) below which no key can be selected
+    uint32_t warp_cnt[kWarps];
+    uint32_t prune_lb;             // lower bound (ord value) below which no key of this CTA can be selected
+    uint32_t sv_count2;            // second counter for compacting the survivor list
     uint32_t sv_count;             // survivors of the pruning pass (may exceed the list capacity: overflow)
 };
 
@@ -120,8 +127,10 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Shared& sh = *reinterpret_cast<Shared*>(smem_raw);
     unsigned long long* sel = reinterpret_cast<unsigned long long*>(smem_raw + ((sizeof(Shared) + 15) / 16) * 16);
-    uint2* sv = reinterpret_cast<uint2*>(sel + cap);          // survivors (ord, idx); `cap` entries iff prune
-    uint32_t* cache = reinterpret_cast<uint32_t*>(sv + (prune ? cap : 0));
+    const int svcap = 4 * cap;                                // entries of each survivor buffer (iff prune)
+    uint2* sv = reinterpret_cast<uint2*>(sel + cap);          // survivors (ord, idx)
+    uint2* sv_alt = sv + (prune ? svcap : 0);                 // compaction target; the two swap roles
+    uint32_t* cache = reinterpret_cast<uint32_t*>(sv + (prune ? 2 * svcap : 0));
 
     // ---- this rank's keys: chunks rank, rank + nc, ... of kChunk consecutive flat indices -------------
     const uint32_t N = (uint32_t)((long long)W_in * C);  // < 2^31 (validated by the API)
@@ -136,7 +145,7 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
     };
 
     for (int b = tid; b < 2 * kBins + 2 * kCoarse; b += kThreads) (&sh.hist[0][0])[b] = 0;  // hist + coarse
-    if (tid == 0) { sh.cursor = 0; sh.prune_bin = 0; sh.sv_count = 0; }
+    if (tid == 0) { sh.cursor = 0; sh.prune_lb = 0; sh.sv_count = 0; sh.sv_count2 = 0; }
 
     // ---- load: the one pass over HBM ---------------------------------------------------
     // All loads of an iteration are issued before any is consumed: indices are clamped instead of branched
@@ -144,11 +153,15 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
     // bm[]: running maxima of 4 disjoint key subsets per thread ("buckets"), used to prune the histograms.
     uint32_t mx = 0u, mn = 0xffffffffu;
     uint32_t bm[4] = {0u, 0u, 0u, 0u};
+    // With pruning, only the keys that fit the cache are loaded here; the rest is streamed ONCE further down,
+    // after a selection bound is known, and only its few survivors are kept.
+    const bool pruning = prune && N > (uint32_t)cap;
+    const int span_c = (pruning && span > cache_cap) ? cache_cap : span;   // keys handled by this first loop
     const bool vec = (N & 3u) == 0 && (!sc || (C & 3) == 0) && ((reinterpret_cast<uintptr_t>(lp) & 15u) == 0) &&
                      (cache_cap & 3) == 0;
     if (vec) {
         // 16-byte loads: 4 consecutive candidates of one parent beam per load, 64 KB in flight per CTA
-        const int span4 = span >> 2;
+        const int span4 = span_c >> 2;
         for (int base4 = 0; base4 < span4; base4 += kThreads * kUnroll) {
             float4 lv[kUnroll];
             float sv[kUnroll];
@@ -162,7 +175,7 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
 #pragma unroll
             for (int x = 0; x < kUnroll; ++x) {
                 const int j = 4 * (base4 + x * kThreads + tid);
-                if (j < span && idx_of(j) < N) {
+                if (j < span_c && idx_of(j) < N) {
                     uint4 o;
                     o.x = ord_of(__fadd_rn(sv[x], lv[x].x)); o.y = ord_of(__fadd_rn(sv[x], lv[x].y));
                     o.z = ord_of(__fadd_rn(sv[x], lv[x].z)); o.w = ord_of(__fadd_rn(sv[x], lv[x].w));
@@ -174,7 +187,7 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
             }
         }
     } else {
-        for (int base = 0; base < span; base += kThreads * kUnroll) {
+        for (int base = 0; base < span_c; base += kThreads * kUnroll) {
             float lv[kUnroll], sv[kUnroll];
 #pragma unroll
             for (int x = 0; x < kUnroll; ++x) {
@@ -186,11 +199,157 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
 #pragma unroll
             for (int x = 0; x < kUnroll; ++x) {
                 const int j = base + x * kThreads + tid;
-                if (j < span && idx_of(j) < N) {
+                if (j < span_c && idx_of(j) < N) {
                     const uint32_t o = ord_of(__fadd_rn(sv[x], lv[x]));
                     if (j < cache_cap) cache[j] = o;
                     mx = max(mx, o); mn = min(mn, o);
                     bm[x & 3] = max(bm[x & 3], o);
+                }
+            }
+        }
+    }
+    // ---- pruning bound (large slices) -----------------------------------------------------------
+    // Shared-memory atomics cost ~1 cycle per key, so a histogram over all keys would dominate.  Any value L such
+    // that at least K of this CTA's keys are >= L is a lower bound of the user's W_out-th key, so this CTA may
+    // drop every key below L (the histograms then miss only keys below the user's threshold: the boundary bin is
+    // still found).  L = lower edge of the 11-bit bin holding the K-th largest of a set of
+    // real keys: first the per-thread bucket maxima of the parked keys, later the survivor list itself.
+    auto block_minmax = [&](uint32_t& vmax, uint32_t& vmin, uint32_t& cnt) {   // block-wide (max, min, sum)
+        vmax = __reduce_max_sync(0xffffffffu, vmax);
+        vmin = __reduce_min_sync(0xffffffffu, vmin);
+        cnt = __reduce_add_sync(0xffffffffu, cnt);
+        if (lane == 0) { sh.warp_max[warp] = vmax; sh.warp_min[warp] = vmin; sh.warp_cnt[warp] = cnt; }
+        __syncthreads();
+        vmax = __reduce_max_sync(0xffffffffu, lane < kWarps ? sh.warp_max[lane] : 0u);
+        vmin = __reduce_min_sync(0xffffffffu, lane < kWarps ? sh.warp_min[lane] : 0xffffffffu);
+        cnt = __reduce_add_sync(0xffffffffu, lane < kWarps ? sh.warp_cnt[lane] : 0u);
+        __syncthreads();                             // (the per-warp slots are reused)
+    };
+    // K-th largest of the values `each` enumerates (>= K of them, all inside [vmin, vmax]), as a bin edge
+    auto kth_bound = [&](auto&& each, uint32_t vmax, uint32_t vmin) -> uint32_t {
+        const int nbl = vmax == vmin ? 0 : 32 - __clz((int)(vmax ^ vmin));
+        const int shl = max(nbl - 11, 0);
+        const uint32_t mkl = nbl >= 32 ? 0xffffffffu : ((1u << nbl) - 1u);
+        for (int b = tid; b < kBins + kCoarse; b += kThreads) (b < kBins ? sh.hist[1][b] : sh.coarse[1][b - kBins]) = 0;
+        __syncthreads();
+        each([&](uint32_t v) { atomicAdd(&sh.hist[1][(v & mkl) >> shl], 1u); });
+        __syncthreads();
+        {
+            const uint4 v = reinterpret_cast<const uint4*>(&sh.hist[1][0])[tid];
+            uint32_t c4 = v.x + v.y + v.z + v.w;
+            c4 += __shfl_xor_sync(0xffffffffu, c4, 1);
+            c4 += __shfl_xor_sync(0xffffffffu, c4, 2);
+            c4 += __shfl_xor_sync(0xffffffffu, c4, 4);
+            if ((lane & 7) == 0) sh.coarse[1][tid >> 3] = c4;
+        }
+        __syncthreads();
+        if (warp == 0) {
+            const uint32_t chi = sh.coarse[1][32 + lane], clo = sh.coarse[1][lane];
+            const uint32_t tot_hi = __reduce_add_sync(0xffffffffu, chi);
+            const bool in_hi = (uint32_t)W_out <= tot_hi;
+            int cbin, fbin; uint32_t rem2, rem3, cnt;
+            warp_select32(in_hi ? chi : clo, in_hi ? (uint32_t)W_out : (uint32_t)W_out - tot_hi, cbin, rem2, cnt);
+            const int coarse_bin = (in_hi ? 32 : 0) + cbin;
+            warp_select32(sh.hist[1][coarse_bin * 32 + lane], rem2, fbin, rem3, cnt);
+            if (lane == 0) sh.prune_lb = (vmax & ~mkl) | ((uint32_t)(coarse_bin * 32 + fbin) << shl);
+        }
+        __syncthreads();                             // (hist[1] / coarse[1] are re-zeroed during pass 0)
+        return sh.prune_lb;
+    };
+    uint32_t ord_lb = 0u;
+    if (pruning) {
+        uint32_t bx = max(max(bm[0], bm[1]), max(bm[2], bm[3])), bn = 0xffffffffu, nv = 0;
+#pragma unroll
+        for (int b = 0; b < 4; ++b)
+            if (bm[b]) { bn = min(bn, bm[b]); ++nv; }
+        block_minmax(bx, bn, nv);
+        if (nv >= (uint32_t)W_out)                   // (block-uniform)
+            ord_lb = kth_bound([&](auto&& put) {
+#pragma unroll
+                for (int b = 0; b < 4; ++b)
+                    if (bm[b]) put(bm[b]);
+            }, bx, bn);
+    }
+    // ---- the keys beyond the cache: streamed ONCE; only those above the bound are kept, and the bound is
+    // re-tightened from the survivor list itself whenever that fills up (a streaming top-K) -----------------
+    const bool tail_streamed = pruning && span > cache_cap;
+    bool tail_ok = true;                             // false: survivors were lost, fall back to re-reading
+    if (tail_streamed) {
+        const int batch = kThreads * kUnroll * (vec ? 4 : 1);
+        int since_check = 0;
+        for (int base = cache_cap; base < span; base += batch) {
+            auto keep = [&](uint32_t o, uint32_t idx) {
+                mx = max(mx, o); mn = min(mn, o);
+                if (tail_ok && o >= ord_lb) {        // rare: K-ish keys per user
+                    const uint32_t pos = atomicAdd(&sh.sv_count, 1u);
+                    if (pos < (uint32_t)svcap) sv[pos] = make_uint2(o, idx);
+                }
+            };
+            if (vec) {
+                float4 lv[kUnroll];
+                float sv1[kUnroll];
+                uint32_t ib[kUnroll];
+#pragma unroll
+                for (int x = 0; x < kUnroll; ++x) {
+                    const int j = base + 4 * (x * kThreads + tid);
+                    ib[x] = j < span ? idx_of(j) : N;
+                    const uint32_t idc = min(ib[x], N - 4);
+                    const int row = c_shift >= 0 ? (int)(idc >> c_shift) : (int)(idc / (uint32_t)C);
+                    lv[x] = __ldg(reinterpret_cast<const float4*>(lp + idc));
+                    sv1[x] = sc ? __ldg(sc + row) : 0.f;
+                }
+#pragma unroll
+                for (int x = 0; x < kUnroll; ++x) {
+                    if (ib[x] < N) {
+                        keep(ord_of(__fadd_rn(sv1[x], lv[x].x)), ib[x]);
+                        keep(ord_of(__fadd_rn(sv1[x], lv[x].y)), ib[x] + 1);
+                        keep(ord_of(__fadd_rn(sv1[x], lv[x].z)), ib[x] + 2);
+                        keep(ord_of(__fadd_rn(sv1[x], lv[x].w)), ib[x] + 3);
+                    }
+                }
+            } else {
+                float lv[kUnroll], sv1[kUnroll];
+                uint32_t ib[kUnroll];
+#pragma unroll
+                for (int x = 0; x < kUnroll; ++x) {
+                    const int j = base + x * kThreads + tid;
+                    ib[x] = j < span ? idx_of(j) : N;
+                    const uint32_t idc = min(ib[x], N - 1);
+                    const int row = c_shift >= 0 ? (int)(idc >> c_shift) : (int)(idc / (uint32_t)C);
+                    lv[x] = __ldg(lp + idc);
+                    sv1[x] = sc ? __ldg(sc + row) : 0.f;
+                }
+#pragma unroll
+                for (int x = 0; x < kUnroll; ++x)
+                    if (ib[x] < N) keep(ord_of(__fadd_rn(sv1[x], lv[x])), ib[x]);
+            }
+            // the list is inspected every 4th batch only: a block barrier per batch would stop the warps from
+            // overlapping each other's load latency (measured 2x on the whole stream)
+            if (++since_check < 4 && base + batch < span) continue;
+            since_check = 0;
+            __syncthreads();
+            const uint32_t cnt = sh.sv_count;        // (block-uniform)
+            __syncthreads();                         // everyone has read it before the next batch appends
+            if (tail_ok && cnt > (uint32_t)(svcap / 2)) {
+                if (cnt > (uint32_t)svcap) {
+                    tail_ok = false;                 // entries were dropped
+                } else {                             // re-tighten: K-th largest survivor, then compact the list
+                    uint32_t bx = 0u, bn = 0xffffffffu, nv = 0;
+                    for (uint32_t e = tid; e < cnt; e += kThreads) { bx = max(bx, sv[e].x); bn = min(bn, sv[e].x); ++nv; }
+                    block_minmax(bx, bn, nv);
+                    const uint32_t nl = kth_bound([&](auto&& put) {
+                        for (uint32_t e = tid; e < cnt; e += kThreads) put(sv[e].x);
+                    }, bx, bn);
+                    ord_lb = max(ord_lb, nl);
+                    for (uint32_t e = tid; e < cnt; e += kThreads)
+                        if (sv[e].x >= ord_lb) sv_alt[atomicAdd(&sh.sv_count2, 1u)] = sv[e];
+                    __syncthreads();
+                    const uint32_t c2 = sh.sv_count2;
+                    __syncthreads();
+                    if (tid == 0) { sh.sv_count = c2; sh.sv_count2 = 0; }
+                    uint2* t2 = sv; sv = sv_alt; sv_alt = t2;
+                    if (c2 > (uint32_t)(svcap / 2)) tail_ok = false;       // ties: the list cannot shrink
+                    __syncthreads();
                 }
             }
         }
@@ -228,7 +387,7 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
     // Walk ALL keys of this rank, warp-uniformly: fn(valid, ord, idx).  Parked keys come from shared memory,
     // 4 in flight per thread; keys beyond the cache are recomputed from global memory (L2) with the same
     // batched, branch-free loads as the first pass.
-    auto scan_all = [&](auto&& fn) {
+    auto scan_cached = [&](auto&& fn) {
         const int n_c = min(span, cache_cap);
         for (int base = 0; base < n_c; base += kThreads * 4) {
             uint32_t o4[4], i4[4];
@@ -241,6 +400,9 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
 #pragma unroll
             for (int x = 0; x < 4; ++x) fn(i4[x] < N, o4[x], i4[x]);
         }
+    };
+    auto scan_all = [&](auto&& fn) {
+        scan_cached(fn);
         if (span <= cache_cap) return;
         if (vec) {
             for (int base4 = cache_cap >> 2; base4 < (span >> 2); base4 += kThreads * 4) {
@@ -293,42 +455,10 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
     int r = nb + nbi;                 // unresolved low bits of V (<= 63)
     uint32_t cb = N;                  // candidates (= keys with V >> r == pref)
 
-    // ---- pruning bound (large slices): shared-memory atomics cost ~1 cycle per key, so a histogram over
-    // all keys would dominate.  Each thread kept the maxima of 4 disjoint subsets of its keys; if K of this
-    // CTA's 2048 bucket maxima lie in first-pass bins >= b, at least K real keys do, so the W_out-th key of
-    // the whole user cannot lie below bin b.  Every CTA may drop its keys below its own b: the cluster-wide
-    // boundary bin found from the pruned histograms is >= every CTA's b, and exact from there upwards.
-    bool pruning = prune && N > (uint32_t)cap && r > 0;
-    if (pruning) {
-        const int w0 = min(11, r), shift0 = r - w0;
-#pragma unroll
-        for (int b = 0; b < 4; ++b)
-            if (bm[b]) atomicAdd(&sh.hist[1][(uint32_t)((((unsigned long long)(bm[b] & lowmask)) << nbi) >> shift0)], 1u);
-        __syncthreads();
-        {
-            const uint4 v = reinterpret_cast<const uint4*>(&sh.hist[1][0])[tid];
-            uint32_t c4 = v.x + v.y + v.z + v.w;
-            c4 += __shfl_xor_sync(0xffffffffu, c4, 1);
-            c4 += __shfl_xor_sync(0xffffffffu, c4, 2);
-            c4 += __shfl_xor_sync(0xffffffffu, c4, 4);
-            if ((lane & 7) == 0) sh.coarse[1][tid >> 3] = c4;
-        }
-        __syncthreads();
-        if (warp == 0) {
-            const uint32_t chi = sh.coarse[1][32 + lane], clo = sh.coarse[1][lane];
-            const uint32_t tot_hi = __reduce_add_sync(0xffffffffu, chi), tot_lo = __reduce_add_sync(0xffffffffu, clo);
-            if (tot_hi + tot_lo >= K) {             // (fewer buckets than K: no bound)
-                const bool in_hi = K <= tot_hi;
-                int cbin, fbin; uint32_t rem2, rem3, cnt;
-                warp_select32(in_hi ? chi : clo, in_hi ? K : K - tot_hi, cbin, rem2, cnt);
-                const int coarse_bin = (in_hi ? 32 : 0) + cbin;
-                warp_select32(sh.hist[1][coarse_bin * 32 + lane], rem2, fbin, rem3, cnt);
-                if (lane == 0) sh.prune_bin = (uint32_t)(coarse_bin * 32 + fbin);
-            }
-        }
-        __syncthreads();                             // hist[1] / coarse[1] are re-zeroed during pass 0
-    }
-    const uint32_t prune_bin = sh.prune_bin;
+    // Survivor list: the streamed tail's survivors are already in it; the first pass adds the parked keys above
+    // the bound.  If it overflows (heavy ties), every loop falls back to walking all keys (tail re-read via L2).
+    const uint32_t n_tail = tail_streamed ? sh.sv_count : 0u;    // (complete: written before the cluster barrier)
+    if (tail_streamed) __syncthreads();                          // read by everyone before the first pass appends
     bool use_sv = false;                             // later loops walk the survivor list instead of all keys
     uint32_t n_sv = 0;
 #pragma unroll 1
@@ -340,37 +470,35 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
             for (uint32_t e = tid; e < n_sv; e += kThreads) {
                 const uint2 k = sv[e];
                 const unsigned long long v = vkey(k.x, k.y);
-                if ((v >> r) == pref) atomicAdd(&sh.hist[arr][(uint32_t)(v >> shift) & mask], 1u);
+                if (k.x >= ord_lb && (v >> r) == pref) atomicAdd(&sh.hist[arr][(uint32_t)(v >> shift) & mask], 1u);
             }
         } else {
-            if (pruning && pass == 0) {
-                // first pass of a pruned run: nearly every key fails the bound, so the test must be cheap.
-                // While the digit lies wholly inside the ord bits (shift >= nbi) it is a 32-bit shift.
-                const bool narrow = shift >= nbi;
-                const int sh32 = narrow ? shift - nbi : 0;
-                scan_all([&](bool ok, uint32_t o, uint32_t idx) {
-                    if (!ok) return;
-                    uint32_t dg;
-                    if (narrow) dg = (o & lowmask) >> sh32;
-                    else dg = (uint32_t)(vkey(o, idx) >> shift) & mask;
-                    if (dg >= prune_bin) {                   // rare: K-ish keys per user
-                        atomicAdd(&sh.hist[arr][dg], 1u);
+            if (pruning && pass == 0 && tail_ok) {
+                // first pass of a pruned run: nearly every parked key fails the bound (one compare); the few
+                // that pass enter the histogram and join the tail's survivors in the list
+                for (uint32_t e = tid; e < n_tail; e += kThreads) {
+                    const uint2 k = sv[e];
+                    if (k.x >= ord_lb) atomicAdd(&sh.hist[arr][(uint32_t)(vkey(k.x, k.y) >> shift) & mask], 1u);
+                }
+                scan_cached([&](bool ok, uint32_t o, uint32_t idx) {
+                    if (ok && o >= ord_lb) {
+                        atomicAdd(&sh.hist[arr][(uint32_t)(vkey(o, idx) >> shift) & mask], 1u);
                         const uint32_t pos = atomicAdd(&sh.sv_count, 1u);
-                        if (pos < (uint32_t)cap) sv[pos] = make_uint2(o, idx);
+                        if (pos < (uint32_t)svcap) sv[pos] = make_uint2(o, idx);
                     }
                 });
             } else {
                 scan_all([&](bool ok, uint32_t o, uint32_t idx) {
-                    if (!ok) return;
+                    if (!ok || o < ord_lb) return;
                     const unsigned long long v = vkey(o, idx);
                     if ((v >> r) == pref) atomicAdd(&sh.hist[arr][(uint32_t)(v >> shift) & mask], 1u);
                 });
             }
         }
         __syncthreads();
-        if (pruning && pass == 0) {                      // list complete?  else fall back to scanning all keys
+        if (pruning && pass == 0 && tail_ok) {           // list complete?  else fall back to scanning all keys
             n_sv = sh.sv_count;
-            use_sv = n_sv <= (uint32_t)cap;
+            use_sv = n_sv <= (uint32_t)svcap;
         }
         {   // coarse histogram: 32 fine bins = 8 threads x 4 bins
             const uint4 v = reinterpret_cast<const uint4*>(&sh.hist[arr][0])[tid];
@@ -431,7 +559,7 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
     // Now: keys with (V >> r) > pref are selected (K - rem of them); `rem` more come from the `cb` keys with
     // (V >> r) == pref, and (K - rem) + cb <= cap: gather them all, the sort decides inside the boundary bin.
     auto take = [&](bool ok, uint32_t o, uint32_t idx) {
-        const bool f = ok && (vkey(o, idx) >> r) >= pref;
+        const bool f = ok && o >= ord_lb && (vkey(o, idx) >> r) >= pref;
         const uint32_t bal = __ballot_sync(0xffffffffu, f);
         if (bal) {  // one shared-memory atomic per warp-iteration reserves the slots
             const int leader = __ffs(bal) - 1;
@@ -573,7 +701,7 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
     const int cap = next_pow2(W_out) * 2 < 128 ? 128 : next_pow2(W_out) * 2;  // sort buffer entries
     // pruning pays once a thread holds many keys (>= 16: slices of 8192) and needs K <= the 2048 buckets of a CTA
     const int prune = (N / kMaxCluster >= 8192 || N >= 32768) && W_out <= 2048 ? 1 : 0;
-    const size_t fixed = ((sizeof(Shared) + 15) / 16) * 16 + (size_t)cap * 8 * (prune ? 2 : 1);
+    const size_t fixed = ((sizeof(Shared) + 15) / 16) * 16 + (size_t)cap * 8 * (prune ? 9 : 1);  // sel + 2 lists of 4 * cap
     const long long cache_max = ((long long)kSmemBudget - (long long)fixed) / 4;
     static bool attr_done = false;  // idempotent; a benign race at worst repeats the calls
     if (!attr_done) {

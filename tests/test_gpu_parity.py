@@ -20,7 +20,7 @@ def test_teacher_forced_parity(name):
     assert any(r[0] == "topk" for r in rep) and any(r[0] == "attn" for r in rep)
 
 
-@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5"])
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5", "paper_b1"])
 def test_full_size_parity(name):
     """BASELINE.json's full sizes in bench.py's launch configuration (DecodePass under CUDA-graph replay):
     all selections bit-exact, append bitwise, sampled attention rows within tolerance."""

@@ -83,3 +83,17 @@ def test_slice_larger_than_cache():
     score = r.normal(-5, 1, (1, 128)).astype(np.float32)
     _check(logp, score, 1024)
     _check((np.round(logp * 4) / 4).astype(np.float32), (np.round(score * 4) / 4).astype(np.float32), 1024)
+
+
+def test_streamed_tail_with_sorted_parent_scores():
+    """The realistic large case: parent scores arrive sorted (best beams first), slices are larger than the
+    cache, so the tail is streamed once against a bound that is re-tightened from the survivor list; also with a
+    late burst (the best parent LAST), which overflows the list and takes the fallback."""
+    r = _rng(5)
+    logits = r.normal(0, 2, (2, 128, 8192))
+    logp = (logits - np.log(np.exp(logits).sum(-1, keepdims=True))).astype(np.float32)
+    score = np.sort(r.normal(-8, 2, (2, 128)).astype(np.float32))[:, ::-1].copy()
+    _check(logp, score, 512)
+    _check(logp, score[:, ::-1].copy(), 512)
+    score2 = score.copy(); score2[:, -1] = 5.0
+    _check(logp, score2, 300)
