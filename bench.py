@@ -3,7 +3,8 @@
 
 A "step" = one whole pass of the hot path over one batch of
 BASELINE.json configs[1] ("cfg2"): decode steps t = 0,1,2, each
-    stark_kv_append_reorg (t>=1) -> stark_prefix_attn -> stark_tree_attn_step -> stark_beam_topk.
+    bf16: stark_decode_step (A4 + A1 + A2 in one launch) -> stark_beam_topk
+    fp32: stark_kv_append_reorg (t>=1) -> stark_prefix_attn -> stark_tree_attn_step -> stark_beam_topk.
 metric = generated SIDs/s (B * W_d final beams per pass / pass time); also us per decode step.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl stark|reference] [--workload cfg2]
@@ -429,7 +430,16 @@ def run_stark(args, cfg):
     kern = {}
     it = 40 * R
     for t in range(cfg.d):
-        if passes[0].fused:
+        if passes[0].inline_append:      # stark_decode_step: the level's append rides inside the attention launch
+            fl, by = work_decode(cfg, lens, nq[t], t)
+            if t >= 1:
+                by += work_append(cfg, nq[t])
+            us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.step(t, p.q[t], p.k_new[t] if t else None,
+                                                                        p.v_new[t] if t else None,
+                                                                        p.sel[t - 1][1] if t else None, out=p.out[t]))
+                                         for p in passes], it, use_graph)
+            kern[f"decode_step.t{t}"] = {"us": us, "bytes": by, "flops": fl}
+        elif passes[0].fused:
             fl, by = work_decode(cfg, lens, nq[t], t)
             us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.attend(t, p.q[t], out=p.out[t], fused=True))
                                          for p in passes], it, use_graph)
@@ -445,7 +455,7 @@ def run_stark(args, cfg):
         us = time_graph_loop(torch, [(lambda p=p, t=t: beam_topk(p.logp[t], p.sel[t - 1][0] if t else None, widths[t],
                                                                   out=p.sel[t])) for p in passes], it, use_graph)
         kern[f"beam_topk.t{t}"] = {"us": us, "bytes": work_topk(cfg, w_in, widths[t])}
-        if t >= 1:
+        if t >= 1 and not passes[0].inline_append:
             us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.append(t, p.k_new[t], p.v_new[t], p.sel[t - 1][1]))
                                          for p in passes], it, use_graph)
             kern[f"kv_append_reorg.t{t}"] = {"us": us, "bytes": work_append(cfg, nq[t])}

@@ -196,6 +196,34 @@ int stark_decode_attn(const stark_shape_t* shape, const void* q, int n_q, int le
                       const void* v_suffix, const int32_t* anc, void* out, void* stream);
 
 /* ---------------------------------------------------------------------------
+ * A4 + A1 + A2 fused: one whole decode step of a layer in ONE launch
+ *
+ * Same result, in `out`, in level `level` of k_suffix / v_suffix and in
+ * anc[level&1], as
+ *     stark_kv_append_reorg(shape, level, n_q, k_new, v_new, parent,
+ *                           k_suffix, v_suffix, write_anc ? anc : NULL)
+ *     stark_decode_attn(shape, q, n_q, level, ..., k_suffix, v_suffix, anc, out)
+ * (PAPER.md:263-268 and 284-286).  A query's own K/V row is read from k_new /
+ * v_new, its ancestors' slots from the PREVIOUS level's index through `parent`
+ * (anc[(level-1)&1][u][parent[u,i]][0..level-2]), so nothing this launch writes
+ * is read by it: the append is done by warps of the attention kernel that are
+ * otherwise idle, and the step costs one launch instead of two.
+ *
+ * level 0 (the root queries its prefix) appends nothing: k_new, v_new, parent,
+ * k_suffix, v_suffix and anc may be NULL.  level >= 1: all of them are needed,
+ * except parent at level 1.  write_anc = 0 for layers > 0 of a decoder (the
+ * tree is shared, layer 0 extends the index; `parent` is still read).
+ * k_new, v_new  in [B, n_q, Hkv, D];  parent in [B, n_q] int32;  the rest as in
+ * the separate calls.  bf16 only (UNSUPPORTED for fp32: compose the calls).
+ * Errors: INVALID_ARG, UNSUPPORTED, CUDA.
+ */
+int stark_decode_step(const stark_shape_t* shape, const void* q, int n_q, int level,
+                      const void* k_prefix, const void* v_prefix, const int32_t* cu_seqlens,
+                      int total_tokens, int max_prefix_len, const void* k_new,
+                      const void* v_new, const int32_t* parent, void* k_suffix, void* v_suffix,
+                      int32_t* anc, int write_anc, void* out, void* stream);
+
+/* ---------------------------------------------------------------------------
  * A3. Per-level beam selection
  *
  * Beam score = sum of per-level log-probabilities (Eq. 1);

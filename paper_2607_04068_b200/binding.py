@@ -19,7 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libstark.so")
 STARK_F32, STARK_BF16 = 0, 1
 CALL_PREFIX_ATTN, CALL_TREE_ATTN_STEP, CALL_BEAM_TOPK, CALL_KV_APPEND_REORG = 0, 1, 2, 3
 EXPORTS = (
-    "stark_prefix_attn", "stark_prefix_attn_plan", "stark_tree_attn_step", "stark_decode_attn", "stark_beam_topk",
+    "stark_prefix_attn", "stark_prefix_attn_plan", "stark_tree_attn_step", "stark_decode_attn", "stark_decode_step",
+    "stark_beam_topk",
     "stark_kv_append_reorg", "stark_workspace_bytes", "stark_suffix_bytes",
     "stark_anc_bytes", "stark_version", "stark_status_string", "stark_last_cuda_error",
     "stark_calib_empty", "stark_calib_stream_read",
@@ -65,6 +66,9 @@ def lib() -> ctypes.CDLL:
     L.stark_decode_attn.restype = c_int
     L.stark_decode_attn.argtypes = [P, c_void_p, c_int, c_int, c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p,
                                     c_void_p, c_void_p, c_void_p, c_void_p]
+    L.stark_decode_step.restype = c_int
+    L.stark_decode_step.argtypes = [P, c_void_p, c_int, c_int, c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p,
+                                    c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_void_p]
     L.stark_beam_topk.restype = c_int
     L.stark_beam_topk.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p,
                                   c_void_p, c_size_t, c_void_p]
@@ -152,6 +156,18 @@ def stark_decode_attn(shape: Shape, q: torch.Tensor, n_q: int, level: int, k_pre
     _check(lib().stark_decode_attn(byref(shape), _ptr(q), n_q, level, _ptr(k_prefix), _ptr(v_prefix),
                                    _ptr(cu_seqlens), total_tokens, max_prefix_len, _ptr(k_suffix), _ptr(v_suffix),
                                    _ptr(anc), _ptr(out), _stream()), "stark_decode_attn")
+
+
+def stark_decode_step(shape: Shape, q: torch.Tensor, n_q: int, level: int, k_prefix: torch.Tensor,
+                      v_prefix: torch.Tensor, cu_seqlens: torch.Tensor, total_tokens: int, max_prefix_len: int,
+                      k_new: Optional[torch.Tensor], v_new: Optional[torch.Tensor], parent: Optional[torch.Tensor],
+                      k_suffix: Optional[torch.Tensor], v_suffix: Optional[torch.Tensor],
+                      anc: Optional[torch.Tensor], write_anc: bool, out: torch.Tensor) -> None:
+    """A4 + A1 + A2 fused (bf16): append of the level's K/V and index rows inside the attention launch."""
+    _check(lib().stark_decode_step(byref(shape), _ptr(q), n_q, level, _ptr(k_prefix), _ptr(v_prefix),
+                                   _ptr(cu_seqlens), total_tokens, max_prefix_len, _ptr(k_new), _ptr(v_new),
+                                   _ptr(parent), _ptr(k_suffix), _ptr(v_suffix), _ptr(anc), int(bool(write_anc)),
+                                   _ptr(out), _stream()), "stark_decode_step")
 
 
 def stark_beam_topk(logp: torch.Tensor, score: Optional[torch.Tensor], B: int, W_in: int, C: int, W_out: int,

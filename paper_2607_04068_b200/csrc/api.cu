@@ -221,6 +221,30 @@ int stark_decode_attn(const stark_shape_t* shape, const void* q, int n_q, int le
                                (cudaStream_t)stream);
 }
 
+int stark_decode_step(const stark_shape_t* shape, const void* q, int n_q, int level, const void* k_prefix,
+                      const void* v_prefix, const int32_t* cu_seqlens, int total_tokens, int max_prefix_len,
+                      const void* k_new, const void* v_new, const int32_t* parent, void* k_suffix, void* v_suffix,
+                      int32_t* anc, int write_anc, void* out, void* stream) {
+    int rc = check_shape(shape);
+    if (rc != STARK_OK) return rc;
+    if (!q || !cu_seqlens || !out) return STARK_ERR_INVALID_ARG;
+    if (n_q < 1 || total_tokens < 0 || max_prefix_len < 1 || level < 0 || level > shape->d) return STARK_ERR_INVALID_ARG;
+    if (total_tokens > 0 && (!k_prefix || !v_prefix)) return STARK_ERR_INVALID_ARG;
+    if (level >= 1 && (!k_new || !v_new || !k_suffix || !v_suffix || !anc || n_q > shape->Wmax)) return STARK_ERR_INVALID_ARG;
+    if (level >= 2 && !parent) return STARK_ERR_INVALID_ARG;
+    const Dims p = make_dims(shape);
+    if (!prefix_tc_supported(p, shape->dtype, n_q) || total_tokens < 1) return STARK_ERR_UNSUPPORTED;
+    rc = check_device();
+    if (rc != STARK_OK) return rc;
+    const size_t half = (size_t)p.B * p.Wmax * p.d;
+    const int32_t* anc_prev = level >= 1 ? anc + (size_t)((level - 1) & 1) * half : nullptr;
+    int32_t* anc_new = (level >= 1 && write_anc) ? anc + (size_t)(level & 1) * half : nullptr;
+    return launch_decode_fused(p, q, n_q, level, k_prefix, v_prefix, cu_seqlens, total_tokens,
+                               plan_cluster_splits(p, n_q, max_prefix_len), k_suffix, v_suffix, anc_prev, out,
+                               (cudaStream_t)stream, level >= 1 ? k_new : nullptr, level >= 1 ? v_new : nullptr, parent,
+                               anc_new);
+}
+
 int stark_calib_empty(void* stream) {
     const int rc = check_device();
     if (rc != STARK_OK) return rc;

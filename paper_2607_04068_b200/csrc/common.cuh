@@ -98,7 +98,8 @@ bool prefix_tc_supported(const Dims& p, int dtype, int n_q);
 bool prefix_tc_parity(const Dims& p, int n_q, int n_splits);
 int launch_decode_fused(const Dims& p, const void* q, int n_q, int level, const void* k, const void* v,
                         const int32_t* cu, int total_tokens, int n_splits, const void* ks, const void* vs,
-                        const int32_t* anc_level, void* out, cudaStream_t st);
+                        const int32_t* anc_level, void* out, cudaStream_t st, const void* kn = nullptr,
+                        const void* vn = nullptr, const int32_t* parent = nullptr, int32_t* anc_new = nullptr);
 int launch_tree_attn(const Dims& p, int dtype, const void* q, int n_q, int level, const void* ks,
                      const void* vs, const int32_t* anc, const float* pm, const float* pl,
                      const float* po, int n_splits, void* out, cudaStream_t st);

@@ -194,6 +194,13 @@ struct FusedArgs {
     __nv_bfloat16* out;        // [B, n_q, Hq, D]
     int level, Wmax, d;
     float scale;               // softmax scale (natural units)
+    // stark_decode_step (A4 folded into the same launch), kn != nullptr: this level's own K/V rows are read from
+    // kn / vn [B, n_q, Hkv, D], `anc` is the PREVIOUS level's half and each row's chain is its parent's chain plus
+    // itself; the otherwise idle warps of warpgroup 0 copy kn / vn into the suffix level and write anc_new.
+    const __nv_bfloat16* kn;
+    const __nv_bfloat16* vn;
+    const int32_t* parent;     // [B, n_q] (unused at level 1)
+    int32_t* anc_new;          // this level's half of the ancestor index, or nullptr (layers > 0)
 };
 
 __device__ __forceinline__ void cluster_sync_all() {
@@ -237,12 +244,22 @@ __device__ __forceinline__ void chain_scores(const FusedArgs& fa, float scale_lo
     const uint4* qp = reinterpret_cast<const uint4*>(fa.q + (((size_t)u * n_q + i) * Hq + h) * D);
 #pragma unroll
     for (int c = 0; c < D / 8; ++c) qv[c] = __ldg(qp + c);
+    const bool inl = fa.kn != nullptr;
+    int chain_of = i;                                   // whose row of `anc` holds this query's ancestors
+    if (inl && fa.level >= 2) chain_of = min(max(__ldg(fa.parent + (size_t)u * n_q + i), 0), fa.Wmax - 1);
 #pragma unroll 1
     for (int t = 0; t < fa.level; ++t) {
-        int a = __ldg(fa.anc + ((size_t)u * fa.Wmax + i) * fa.d + t);
-        a = min(max(a, 0), fa.Wmax - 1);                // memory safety on garbage input
-        const size_t off = (size_t)t * level_stride + (((size_t)u * fa.Wmax + a) * Hkv + kv) * D;
-        const uint4* kp = reinterpret_cast<const uint4*>(fa.ks + off);
+        size_t off;
+        const uint4* kp;
+        if (inl && t == fa.level - 1) {                 // itself: not yet in the suffix buffers
+            off = (((size_t)u * n_q + i) * Hkv + kv) * D;
+            kp = reinterpret_cast<const uint4*>(fa.kn + off);
+        } else {
+            int a = __ldg(fa.anc + ((size_t)u * fa.Wmax + chain_of) * fa.d + t);
+            a = min(max(a, 0), fa.Wmax - 1);            // memory safety on garbage input
+            off = (size_t)t * level_stride + (((size_t)u * fa.Wmax + a) * Hkv + kv) * D;
+            kp = reinterpret_cast<const uint4*>(fa.ks + off);
+        }
         float dot = 0.f;
 #pragma unroll
         for (int c = 0; c < D / 8; ++c) {
@@ -335,8 +352,9 @@ __device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char*
         for (int t0 = 0; t0 < (live ? level : 0); t0 += 2) {
             const bool two_lv = t0 + 1 < level;
             const float e[2] = {ch_y[t0], two_lv ? ch_y[t0 + 1] : 0.f};
-            const uint4* vp0 = reinterpret_cast<const uint4*>(fa.vs + ch_off[t0]) + c * 4;
-            const uint4* vp1 = reinterpret_cast<const uint4*>(fa.vs + ch_off[two_lv ? t0 + 1 : t0]) + c * 4;
+            const int t1 = two_lv ? t0 + 1 : t0;
+            const uint4* vp0 = reinterpret_cast<const uint4*>(((fa.vn && t0 == level - 1) ? fa.vn : fa.vs) + ch_off[t0]) + c * 4;
+            const uint4* vp1 = reinterpret_cast<const uint4*>(((fa.vn && t1 == level - 1) ? fa.vn : fa.vs) + ch_off[t1]) + c * 4;
             uint4 vv[2][4];
 #pragma unroll
             for (int k4 = 0; k4 < 4; ++k4) { vv[0][k4] = __ldg(vp0 + k4); vv[1][k4] = __ldg(vp1 + k4); }
@@ -598,6 +616,36 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
             }
             umma_commit(bar_done);
         }
+        }
+        else if (FUSED && fa.kn != nullptr && split == 0 && fa.level > 0) {
+        // ===================== inline KV append + index reorganisation (stark_decode_step) =====================
+        // PAPER.md:284-286.  Warps 2 and 3 of the first split: the K/V rows of this CTA's beams and KV head go
+        // into the suffix level; the CTAs of KV head 0 also extend the ancestor index.  Nothing in this launch
+        // reads what is written here (a query's own row comes from kn / vn, its ancestors from lower levels).
+        const int tid = threadIdx.x - 64;
+        const int b0 = tile0 * beams_per_tile, nb = min(n_q, b0 + (parity ? 1 : 2) * beams_per_tile) - b0;
+        constexpr int VPR = D / 8;                       // 16-byte vectors per row
+        const size_t lvl_off = (size_t)(fa.level - 1) * B * fa.Wmax * Hkv * D;
+        const int per = nb * VPR;
+#pragma unroll 2
+        for (int idx = tid; idx < 2 * per; idx += 64) {
+            const int which = idx >= per, rem = idx - which * per, i2 = b0 + rem / VPR, c = rem % VPR;
+            const __nv_bfloat16* src = (which ? fa.vn : fa.kn) + (((size_t)u * n_q + i2) * Hkv + kv) * D;
+            __nv_bfloat16* dst = const_cast<__nv_bfloat16*>(which ? fa.vs : fa.ks) + lvl_off +
+                                 (((size_t)u * fa.Wmax + i2) * Hkv + kv) * D;
+            reinterpret_cast<uint4*>(dst)[c] = __ldg(reinterpret_cast<const uint4*>(src) + c);
+        }
+        if (fa.anc_new != nullptr && kv == 0)
+            for (int bi = tid; bi < nb; bi += 64) {
+                const int i2 = b0 + bi;
+                int32_t* row = fa.anc_new + ((size_t)u * fa.Wmax + i2) * fa.d;
+                if (fa.level >= 2) {
+                    const int par = min(max(__ldg(fa.parent + (size_t)u * n_q + i2), 0), fa.Wmax - 1);
+                    const int32_t* prow = fa.anc + ((size_t)u * fa.Wmax + par) * fa.d;
+                    for (int t2 = 0; t2 < fa.level - 1; ++t2) row[t2] = __ldg(prow + t2);
+                }
+                row[fa.level - 1] = i2;
+            }
         }
         if (FUSED && n_splits > 1) {                     // the two cluster barriers of the fused tail (B1, B2)
             __syncwarp();
@@ -932,7 +980,8 @@ int launch_prefix_tc(const Dims& p, const void* q, int n_q, const void* k, const
 // A1 + A2 in one launch (bf16): n_splits in {1, 2, 4, 8} = cluster size along the prefix.
 int launch_decode_fused(const Dims& p, const void* q, int n_q, int level, const void* k, const void* v,
                         const int32_t* cu, int total_tokens, int n_splits, const void* ks, const void* vs,
-                        const int32_t* anc_level, void* out, cudaStream_t st) {
+                        const int32_t* anc_level, void* out, cudaStream_t st, const void* kn, const void* vn,
+                        const int32_t* parent, int32_t* anc_new) {
     CUtensorMap tq, tk, tv;
     if (!make_map(&tq, q, p.D, p.Hq, (long long)p.B * n_q, p.G, BM / p.G) ||
         !make_map(&tk, k, p.D, p.Hkv, total_tokens, 1, BN) || !make_map(&tv, v, p.D, p.Hkv, total_tokens, 1, BN)) {
@@ -943,6 +992,7 @@ int launch_decode_fused(const Dims& p, const void* q, int n_q, int level, const 
     fa.q = (const __nv_bfloat16*)q; fa.ks = (const __nv_bfloat16*)ks; fa.vs = (const __nv_bfloat16*)vs;
     fa.anc = anc_level; fa.out = (__nv_bfloat16*)out;
     fa.level = level; fa.Wmax = p.Wmax; fa.d = p.d; fa.scale = p.scale;
+    fa.kn = (const __nv_bfloat16*)kn; fa.vn = (const __nv_bfloat16*)vn; fa.parent = parent; fa.anc_new = anc_new;
     if (p.D == 128) return launch_fused_d<128>(p, tq, tk, tv, n_q, cu, n_splits, fa, st);
     return launch_fused_d<64>(p, tq, tk, tv, n_q, cu, n_splits, fa, st);
 }

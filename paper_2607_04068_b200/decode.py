@@ -76,6 +76,18 @@ class StarkLayer:
             self.tree(level, q, out, anc)
         return out
 
+    def step(self, level: int, q: torch.Tensor, k_new: Optional[torch.Tensor], v_new: Optional[torch.Tensor],
+             parent: Optional[torch.Tensor], out: Optional[torch.Tensor] = None,
+             anc: Optional[torch.Tensor] = None, write_anc: bool = True) -> torch.Tensor:
+        """append(level, k_new, v_new, parent) + attend(level, q) in ONE launch (stark_decode_step, bf16 only).
+        `anc` = another layer's index buffer (the tree is shared: pass write_anc=False for layers > 0)."""
+        if out is None:
+            out = torch.empty_like(q)
+        sb.stark_decode_step(self.shape, q, int(q.shape[1]), level, self.k_prefix, self.v_prefix, self.cu,
+                             self.total_tokens, self.max_len, k_new, v_new, parent, self.k_suffix, self.v_suffix,
+                             self.anc if anc is None else anc, write_anc, out)
+        return out
+
     def n_splits(self, n_q: int) -> int:
         return self._partials(n_q)[0]
 

@@ -1,6 +1,7 @@
 """One whole pass of the STARK hot path (all rows of SURVEY.md section 8(a)) for one batch:
-decode steps t = 0..d-1, each  append(t>=1) -> decode attention -> beam_topk, where decode attention is
-the fused stark_decode_attn launch for bf16 and stark_prefix_attn -> stark_tree_attn_step for fp32.
+decode steps t = 0..d-1, each  append(t>=1) -> decode attention -> beam_topk.  bf16: append and attention are
+ONE launch (stark_decode_step; `inline_append=False` keeps stark_kv_append_reorg -> stark_decode_attn); fp32:
+stark_kv_append_reorg -> stark_prefix_attn -> stark_tree_attn_step.
 
 Inputs (prefix K/V, per-step q / k_new / v_new, per-level log-probs) are device tensors;
 `DecodePass.run()` only enqueues library calls on the current stream, so a pass is CUDA-graph
@@ -20,10 +21,11 @@ class DecodePass:
     def __init__(self, B: int, Hq: int, Hkv: int, D: int, d: int, C: int, widths: List[int], dtype: torch.dtype,
                  k_prefix: torch.Tensor, v_prefix: torch.Tensor, cu_seqlens: torch.Tensor, max_prefix_len: int,
                  q: List[torch.Tensor], k_new: List[torch.Tensor], v_new: List[torch.Tensor],
-                 logp: List[torch.Tensor]):
+                 logp: List[torch.Tensor], inline_append: bool = True):
         self.B, self.d, self.C, self.widths = B, d, C, list(widths)
         self.n_q = [1] + self.widths                      # queries per user at step t
         self.fused = dtype == torch.bfloat16 and int(k_prefix.shape[0]) > 0
+        self.inline_append = self.fused and inline_append
         self.layer = StarkLayer(B, Hq, Hkv, D, d, max(self.widths), dtype, k_prefix, v_prefix, cu_seqlens,
                                 max_prefix_len, n_q_per_step=None if self.fused else self.n_q[:d])
         self.q, self.k_new, self.v_new, self.logp = q, k_new, v_new, logp
@@ -34,16 +36,21 @@ class DecodePass:
                      torch.empty((B, w), dtype=torch.int32, device=dev)) for w in self.widths]
 
     #: library kernels launched by one run(): attention (1 fused or 2) + top-k per step, + append for t >= 1
+    #: unless it rides inside the attention launch
     @property
     def launches(self) -> int:
-        return (2 if self.fused else 3) * self.d + (self.d - 1)
+        return (2 if self.fused else 3) * self.d + (0 if self.inline_append else self.d - 1)
 
     def run(self) -> None:
         score = parent = None
         for t in range(self.d):
-            if t >= 1:
-                self.layer.append(t, self.k_new[t], self.v_new[t], parent)
-            self.layer.attend(t, self.q[t], out=self.out[t], fused=self.fused)
+            if self.inline_append:
+                self.layer.step(t, self.q[t], self.k_new[t] if t >= 1 else None, self.v_new[t] if t >= 1 else None,
+                                parent, out=self.out[t])
+            else:
+                if t >= 1:
+                    self.layer.append(t, self.k_new[t], self.v_new[t], parent)
+                self.layer.attend(t, self.q[t], out=self.out[t], fused=self.fused)
             score, parent, _ = beam_topk(self.logp[t], score, self.widths[t], out=self.sel[t])
 
     def result(self) -> Dict[str, List[torch.Tensor]]:

@@ -1,7 +1,7 @@
 """Config 3 harness (BASELINE.json configs[2]; reading R17): a random-init decoder-only transformer
 whose GEMMs run in torch/cuBLAS while decode attention, KV append/reorg and beam top-k go through the STARK
 library.  TEST INFRASTRUCTURE: it shows the four calls inside a real multi-layer decode loop (the tree is
-shared by all layers: layer 0 writes the ancestor index, the others pass anc = NULL) and captures per-call
+shared by all layers: layer 0 writes the ancestor index, the others pass write_anc = 0) and captures per-call
 inputs so that tests can compare sampled (layer, user, step) triples with the oracle.
 
 Model (R17): token embedding + learned absolute positions for the prefix; SID embedding table [d*C, d_model]
@@ -108,9 +108,9 @@ class Decoder:
             for li, (lw, layer) in enumerate(zip(self.layers, layers)):
                 q, k, v = self._qkv(lw, x)
                 q, k, v = q.contiguous(), k.contiguous(), v.contiguous()
-                if t >= 1:   # the tree is shared by all layers: only layer 0 extends the ancestor index
-                    layer.append(t, k, v, parent, write_anc=(li == 0))
-                o = layer.attend(t, q, anc=layers[0].anc)
+                # append + attention in one launch; the tree is shared by all layers: only layer 0 extends the index
+                o = layer.step(t, q, k if t >= 1 else None, v if t >= 1 else None, parent, anc=layers[0].anc,
+                               write_anc=(li == 0))
                 if capture:
                     cq.append(q), ck.append(k), cv.append(v), co.append(o)
                 x = self._ffn(lw, x + o.reshape(*x.shape[:-1], -1) @ lw["out"])
@@ -131,7 +131,6 @@ class Decoder:
         score = parent = None
         for t in range(sh.d):
             for li, layer in enumerate(layers):
-                if t >= 1:
-                    layer.append(t, cap["k"][t][li], cap["v"][t][li], parent, write_anc=(li == 0))
-                layer.attend(t, cap["q"][t][li], out=cap["out"][t][li], anc=layers[0].anc)
+                layer.step(t, cap["q"][t][li], cap["k"][t][li] if t >= 1 else None, cap["v"][t][li] if t >= 1 else None,
+                           parent, out=cap["out"][t][li], anc=layers[0].anc, write_anc=(li == 0))
             score, parent, _ = beam_topk(cap["logp"][t], score, cap["sel"][t][1].shape[1], out=cap["sel"][t])

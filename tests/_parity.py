@@ -72,6 +72,8 @@ def run_teacher_forced(cfg, seed=0, final_step=True):
     tr = oracle_traces(cfg, dr, final_step=final_step)
     layer = make_layer(cfg, dr)
     dt = torch_dtype(cfg)
+    # a second layer takes every step through the single-launch boundary (stark_decode_step, bf16 only)
+    layer_s = make_layer(cfg, dr) if cfg.dtype == "bf16" else None
     tol = TOL[cfg.dtype]
     report = []
     score = parent = None
@@ -81,13 +83,26 @@ def run_teacher_forced(cfg, seed=0, final_step=True):
         if t >= 1:
             kn = np.stack([tr[u].k_new[t] for u in range(cfg.B)]).astype(np.float32)
             vn = np.stack([tr[u].v_new[t] for u in range(cfg.B)]).astype(np.float32)
-            layer.append(t, to_dev(kn, dt), to_dev(vn, dt), parent)
+            kn, vn = to_dev(kn, dt), to_dev(vn, dt)
+            layer.append(t, kn, vn, parent)
+        else:
+            kn = vn = None
         ref = np.stack([tr[u].attn_out[t] for u in range(cfg.B)])
         # both boundaries: A1 then A2 (partials through HBM), and the fused single launch (bf16 only)
         for what, fused in (("attn", False),) + ((("attn_fused", True),) if cfg.dtype == "bf16" else ()):
             out = layer.attend(t, q, fused=fused).float().cpu().numpy().astype(np.float64)
             err = np.abs(out - ref).max() / np.abs(ref).max()
             report.append((what, t, bool(np.isfinite(out).all() and err <= tol), f"rel_err={err:.3e} tol={tol}"))
+        if layer_s is not None:
+            out = layer_s.step(t, q, kn, vn, parent).float().cpu().numpy().astype(np.float64)
+            err = np.abs(out - ref).max() / np.abs(ref).max()
+            report.append(("attn_step", t, bool(np.isfinite(out).all() and err <= tol), f"rel_err={err:.3e} tol={tol}"))
+            if t >= 1:   # the inline append left the same suffix rows and index rows as stark_kv_append_reorg
+                n = q.shape[1]
+                same = (torch.equal(layer_s.k_suffix[t - 1][:, :n], layer.k_suffix[t - 1][:, :n])
+                        and torch.equal(layer_s.v_suffix[t - 1][:, :n], layer.v_suffix[t - 1][:, :n])
+                        and torch.equal(layer_s.anc[t & 1, :, :n, :t], layer.anc[t & 1, :, :n, :t]))
+                report.append(("step_append_state", t, bool(same), ""))
         if t == cfg.d:
             break
         logp = np.stack([tr[u].logp[t] for u in range(cfg.B)])            # fp32, the oracle's O3 output

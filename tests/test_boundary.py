@@ -71,6 +71,14 @@ def test_validation_before_cuda(L):
     assert L.stark_decode_attn(ctypes.byref(bf), p, 9, 1, p, p, p, 4, 4, p, p, p, p, None) == -1      # n_q > Wmax
     assert L.stark_decode_attn(ctypes.byref(bf), p, 1, 1, p, p, p, 4, 4, p, p, None, p, None) == -1   # anc missing
     assert L.stark_decode_attn(ctypes.byref(sh), p, 1, 0, p, p, p, 4, 4, p, p, p, p, None) == -2      # fp32
+    # single-launch step: (shape, q, n_q, level, kp, vp, cu, total, max_len, k_new, v_new, parent, ks, vs, anc, w, out, st)
+    step = lambda s, *a: L.stark_decode_step(ctypes.byref(s), *a)
+    assert step(bf, None, 1, 0, p, p, p, 4, 4, None, None, None, None, None, None, 1, p, None) == -1  # q missing
+    assert step(bf, p, 1, 4, p, p, p, 4, 4, p, p, p, p, p, p, 1, p, None) == -1                      # level > d
+    assert step(bf, p, 9, 1, p, p, p, 4, 4, p, p, None, p, p, p, 1, p, None) == -1                   # n_q > Wmax
+    assert step(bf, p, 1, 1, p, p, p, 4, 4, None, p, None, p, p, p, 1, p, None) == -1                # k_new missing
+    assert step(bf, p, 1, 2, p, p, p, 4, 4, p, p, None, p, p, p, 0, p, None) == -1                   # parent missing
+    assert step(sh, p, 1, 0, p, p, p, 4, 4, None, None, None, None, None, None, 1, p, None) == -2    # fp32
     assert L.stark_calib_stream_read(None, 64, p, None) == -1
 
 

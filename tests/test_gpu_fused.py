@@ -29,6 +29,8 @@ def _case(B, Hq, Hkv, D, lens, W, d, seed):
     dev = torch.device("cuda")
     bf = lambda a: torch.from_numpy(a).to(dev).to(torch.bfloat16).contiguous()
     layer = StarkLayer(B, Hq, Hkv, D, d, W, torch.bfloat16, bf(K), bf(V), torch.from_numpy(cu).to(dev), int(lens.max()))
+    # the same steps through stark_decode_step (append inside the attention launch)
+    layer_s = StarkLayer(B, Hq, Hkv, D, d, W, torch.bfloat16, layer.k_prefix, layer.v_prefix, layer.cu, int(lens.max()))
     scale = 1.0 / np.sqrt(D)
     k_lv, v_lv, parents = [], [], []
     for t in range(d + 1):
@@ -40,9 +42,16 @@ def _case(B, Hq, Hkv, D, lens, W, d, seed):
             k_lv.append(kn); v_lv.append(vn); parents.append(par)
             layer.append(t, bf(kn), bf(vn), torch.from_numpy(par).to(dev))
         qd = bf(q)
-        fused = layer.attend(t, qd, fused=True).float().cpu().numpy().astype(np.float64)
-        if tot > 0:
-            pass
+        fused_t = layer.attend(t, qd, fused=True)
+        if t >= 1:
+            step_t = layer_s.step(t, qd, bf(kn), bf(vn), torch.from_numpy(par).to(dev))
+            assert torch.equal(layer_s.k_suffix[t - 1], layer.k_suffix[t - 1]), f"step {t}: inline append K"
+            assert torch.equal(layer_s.v_suffix[t - 1], layer.v_suffix[t - 1]), f"step {t}: inline append V"
+            assert torch.equal(layer_s.anc[t & 1, :, :, :t], layer.anc[t & 1, :, :, :t]), f"step {t}: inline index"
+        else:
+            step_t = layer_s.step(t, qd, None, None, None)
+        assert torch.equal(step_t, fused_t), f"step {t}: stark_decode_step differs from append + stark_decode_attn"
+        fused = fused_t.float().cpu().numpy().astype(np.float64)
         two = layer.attend(t, qd, fused=False).float().cpu().numpy().astype(np.float64)
         assert np.isfinite(fused).all()
         # every row: fused vs two-call (both bf16 outputs of the same fp32-accumulated math)
