@@ -306,7 +306,7 @@ def run_cfg3_decoder(args):
                                  "prefix": sh.prefix, "beam": sh.W, "levels": sh.d, "codebook": sh.C,
                                  "launch": launch, "prefill": "untimed (torch SDPA)"},
                       "library_ms_per_step": ms_lib, "gemm_and_glue_ms_per_step": ms_all - ms_lib,
-                      "library_launches": sh.n_layers * (2 * sh.d - 1) + sh.d}), flush=True)  # attend + append, top-k
+                      "library_launches": sh.n_layers * sh.d + sh.d}), flush=True)  # stark_decode_step per layer, top-k
 
 
 def run_reference(args, cfg):
