@@ -688,6 +688,60 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
     }
 }
 
+// ---- small problems (N <= kSmallMax candidates per user: decode step 0 of a 256-code level) ---------------
+// One CTA per user, no cluster, no radix pass: every candidate's composite (~ord, idx) goes to shared memory,
+// each thread counts how many composites are smaller than its own (shared-memory broadcasts) and the
+// candidates of rank < W_out write their result row directly.  Same order as the general kernel: key
+// descending, flat index ascending (reading R6).
+constexpr int kSmallMax = 512;       // beyond this the N^2 / 2 compares cost more than the radix passes
+constexpr int kSmallThreads = 256;
+
+template <int PER>  // candidates per thread
+__global__ void __launch_bounds__(kSmallThreads)
+topk_small_kernel(const float* __restrict__ logp, const float* __restrict__ score, int W_in, int C, int W_out,
+                  float* __restrict__ out_score, int32_t* __restrict__ out_parent, int32_t* __restrict__ out_code) {
+    __shared__ __align__(16) unsigned long long comp[PER * kSmallThreads];
+    const int u = blockIdx.x, tid = threadIdx.x;
+    const int N = W_in * C;
+    const float* __restrict__ lp = logp + (size_t)u * N;
+    const float* __restrict__ sc = score ? score + (size_t)u * W_in : nullptr;
+    float key[PER];
+    unsigned long long mine[PER];
+    int row[PER], rk[PER];
+#pragma unroll
+    for (int x = 0; x < PER; ++x) {
+        const int idx = min(tid + x * kSmallThreads, N - 1);
+        row[x] = idx / C;
+        key[x] = __ldg(lp + idx);
+    }
+#pragma unroll
+    for (int x = 0; x < PER; ++x) {
+        const int idx = tid + x * kSmallThreads;
+        key[x] = __fadd_rn(sc ? __ldg(sc + row[x]) : 0.f, key[x]);
+        mine[x] = idx < N ? (((unsigned long long)(~ord_of(key[x])) << 32) | (uint32_t)idx) : ~0ull;
+        comp[idx] = mine[x];
+        rk[x] = 0;
+    }
+    __syncthreads();
+    const int N2 = (N + 1) & ~1;                         // (a ragged last pair reads a dead slot: ~0, never smaller)
+#pragma unroll 4
+    for (int i = 0; i < N2; i += 2) {
+        const ulonglong2 c = *reinterpret_cast<const ulonglong2*>(comp + i);  // broadcast
+#pragma unroll
+        for (int x = 0; x < PER; ++x) rk[x] += (int)(c.x < mine[x]) + (int)(c.y < mine[x]);
+    }
+#pragma unroll
+    for (int x = 0; x < PER; ++x) {
+        const int idx = tid + x * kSmallThreads;
+        if (idx < N && rk[x] < W_out) {
+            const size_t o = (size_t)u * W_out + rk[x];
+            out_score[o] = key[x];
+            out_parent[o] = row[x];
+            out_code[o] = idx - row[x] * C;
+        }
+    }
+}
+
 int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
 
 }  // namespace
@@ -698,6 +752,14 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
                 float* out_score, int32_t* out_parent, int32_t* out_code, void*, size_t,
                 cudaStream_t st) {
     const long long N = (long long)W_in * C;
+    if (N <= kSmallMax) {
+        if (N <= kSmallThreads)
+            topk_small_kernel<1><<<B, kSmallThreads, 0, st>>>(logp, score, W_in, C, W_out, out_score, out_parent, out_code);
+        else
+            topk_small_kernel<2><<<B, kSmallThreads, 0, st>>>(logp, score, W_in, C, W_out, out_score, out_parent, out_code);
+        STARK_LAUNCH_CHECK();
+        return STARK_OK;
+    }
     const int cap = next_pow2(W_out) * 2 < 128 ? 128 : next_pow2(W_out) * 2;  // sort buffer entries
     // pruning pays once a thread holds many keys (>= 16: slices of 8192) and needs K <= the 2048 buckets of a CTA
     const int prune = (N / kMaxCluster >= 8192 || N >= 32768) && W_out <= 2048 ? 1 : 0;

@@ -97,3 +97,20 @@ def test_streamed_tail_with_sorted_parent_scores():
     _check(logp, score[:, ::-1].copy(), 512)
     score2 = score.copy(); score2[:, -1] = 5.0
     _check(logp, score2, 300)
+
+
+def test_small_direct_path():
+    """N <= 512 candidates per user (decode step 0 of a 256-code level) take the one-CTA rank-by-counting
+    kernel (1 or 2 candidates per thread): ragged and odd N, N = 256 / 512 exactly, W_out = N, massive ties,
+    signed zeros, -inf; N = 513 .. 1024 sits just above it."""
+    r = _rng(6)
+    for (B, W_in, C, W_out) in [(16, 1, 256, 64), (2, 2, 256, 512), (3, 15, 31, 400), (2, 1, 1, 1), (5, 1, 255, 7),
+                               (2, 19, 27, 513), (2, 4, 256, 1024), (3, 3, 85, 200)]:
+        logp = r.normal(-5, 2, (B, W_in, C)).astype(np.float32)
+        score = None if W_in == 1 else r.normal(-3, 1, (B, W_in)).astype(np.float32)
+        _check(logp, score, W_out)
+        q = (np.round(logp * 2) / 2).astype(np.float32)          # ties everywhere: index order decides
+        _check(q, None if score is None else (np.round(score * 2) / 2).astype(np.float32), W_out)
+    z = np.zeros((2, 4, 128), np.float32); z[0, ::2] = -0.0; z[1, :, 5:] = -np.inf
+    _check(z, None, 100)
+    _check(z, np.zeros((2, 4), np.float32), 512)
