@@ -280,7 +280,9 @@ __device__ __forceinline__ void chain_scores(const FusedArgs& fa, float scale_lo
 // prefix partials of all splits (own rows in TMEM, the others' delivered into the K/V ring), add the suffix
 // chain of each row (Eq. 14: ancestors and itself), normalise, write bf16 rows coalesced.
 // Runs once per CTA, so it is written for SMALL CODE (rolled loops, per-lane scratch in shared memory): a
-// fully unrolled version was instruction-fetch bound (~100 KB of straight-line code: 16 us).
+// fully unrolled version was instruction-fetch bound (~100 KB of straight-line code: 16 us).  The same holds
+// for every once-per-CTA loop over 32-column chunks in this kernel (rescale, in-CTA merge, DSMEM send): rolled,
+// they are worth 1.3 us per config-2 pass, where the kernel's code is re-fetched after every top-k launch.
 template <int D>
 __device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char* smem_raw, uint32_t ring_off, int ob, int me,
                                           int ns, int lane, uint32_t aO, bool has, float m_own, float l_own,
@@ -325,7 +327,7 @@ __device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char*
     const float inv = denom > 0.f ? 1.0f / denom : 0.f;
 
     // ---- output row, 32 columns at a time ---------------------------------------------------------------------
-#pragma unroll 2
+#pragma unroll 1
     for (int c = 0; c < D / 32; ++c) {
         float acc[32];
         {
@@ -701,7 +703,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                     if (__any_sync(0xffffffffu, grow)) {
                         // S_t(j) ready => PV_t(j-1) completed (in-order tensor pipe): O_t is quiescent
                         const float alpha = grow ? fast_exp2(m_ref - m_new) : 1.0f;
-#pragma unroll
+#pragma unroll 1
                         for (int c = 0; c < D / 32; ++c) {
                             uint32_t o[32];
                             tmem_ld32(aO + c * 32, o);
@@ -750,7 +752,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                     tc_fence_after();
                     *mml = make_float2(m_ref, l_sum);
                     if (my_tiles > 0) {
-#pragma unroll
+#pragma unroll 1
                         for (int c = 0; c < D / 32; ++c) {
                             uint32_t o[32];
                             tmem_ld32(aO + c * 32, o);
@@ -770,7 +772,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                         tc_fence_after();
                         const float m = fmaxf(m_ref, ml.x);
                         const float a0 = fast_exp2(m_ref - m), a1 = fast_exp2(ml.x - m);
-#pragma unroll
+#pragma unroll 1
                         for (int c = 0; c < D / 32; ++c) {
                             uint32_t o[32];
                             tmem_ld32(aO + c * 32, o);
@@ -835,7 +837,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 const uint32_t slot = (uint32_t)(ob * n_splits) + me;
                 const uint32_t dst = map_to_rank(sKV + slot * SLOT + (uint32_t)lane * D * 4, (uint32_t)owner);
                 constexpr int CPR = D / 4;
-#pragma unroll
+#pragma unroll 1
                 for (int c = 0; c < D / 32; ++c) {
                     uint32_t o[32];
                     tmem_ld32(aO + c * 32, o);
