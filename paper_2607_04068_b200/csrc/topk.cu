@@ -742,6 +742,213 @@ topk_small_kernel(const float* __restrict__ logp, const float* __restrict__ scor
     }
 }
 
+// ---- medium problems (kSmallMax < N <= kMidMaxN candidates per user, W_out <= kMidMaxK) ---------------------
+// One 1024-thread CTA per user, 16 candidates per thread, no cluster: at these sizes (config 2: 16 K candidates,
+// W_out = 64) the general kernel's time is its chain of cluster barriers and DSMEM pulls, not its data.
+//   1. load once; the order-preserving keys are parked in shared memory (64 KB);
+//   2. bound: if K of the 1024 per-thread maxima lie in 11-bit bins >= b, at least K keys do, so the W_out-th key
+//      cannot lie below bin b (the pruning argument of the general kernel): one tiny histogram of 1024 values;
+//   3. the candidates at or above the bound (normally W_out plus a few) go to a list; each list entry counts the
+//      entries smaller than itself and the ranks < W_out write their result rows -- no sort;
+//   4. more than 1024 survivors (massive ties): exact radix select of the W_out-th key over the parked keys
+//      (up to three 11-bit passes), keys above it plus the lowest-index keys equal to it (index-order prefix
+//      counts) form the list; then step 3's ranking.
+constexpr int kMidThreads = 1024;
+constexpr int kMidKeys = 16;
+constexpr int kMidMaxN = kMidThreads * kMidKeys;
+constexpr int kMidMaxK = 1024;
+
+struct __align__(16) MidShared {
+    uint32_t hist[kBins];
+    uint32_t coarse[kCoarse];          // (directly behind hist: zeroed together)
+    uint32_t wred[2][32];
+    uint32_t sel_bin, sel_rem, sel_cnt, cursor;
+    unsigned long long list[kMidMaxK + 2];
+};
+
+// warp 0: highest bin of sh.hist with suffix count >= rem (requires the total >= rem)
+__device__ __forceinline__ void mid_select(MidShared& sh, uint32_t rem) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t cu = sh.coarse[32 + lane], cl = sh.coarse[lane];
+    uint32_t tot_u = cu;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) tot_u += __shfl_xor_sync(0xffffffffu, tot_u, o);
+    int g, b;
+    uint32_t r2, c2, r3, c3;
+    if (tot_u >= rem) { warp_select32(cu, rem, g, r2, c2); g += 32; }
+    else warp_select32(cl, rem - tot_u, g, r2, c2);
+    warp_select32(sh.hist[32 * g + lane], r2, b, r3, c3);
+    if (lane == 0) { sh.sel_bin = (uint32_t)(32 * g + b); sh.sel_rem = r3; sh.sel_cnt = c3; }
+}
+
+__global__ void __launch_bounds__(kMidThreads, 1)
+topk_mid_kernel(const float* __restrict__ logp, const float* __restrict__ score, int W_in, int C, int c_shift,
+                int W_out, float* __restrict__ out_score, int32_t* __restrict__ out_parent,
+                int32_t* __restrict__ out_code) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint32_t* ords = reinterpret_cast<uint32_t*>(smem_raw);        // [kMidMaxN]
+    __shared__ MidShared sh;
+    const int u = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t N = (uint32_t)(W_in * C), K = (uint32_t)W_out;
+    const float* __restrict__ lp = logp + (size_t)u * N;
+    const float* __restrict__ sc = score ? score + (size_t)u * W_in : nullptr;
+
+    for (int b = tid; b < kBins + kCoarse; b += kMidThreads) sh.hist[b] = 0;   // hist + coarse
+    if (tid == 0) sh.cursor = 0;
+
+    // ---- 1. load: all 16 log-prob loads of a thread in flight at once (one cold round trip); the parent
+    // scores (a few cache lines per user) follow and hit L1 -------------------------------------------------
+    uint32_t tmax = 0u, tmin = 0xffffffffu;
+    {
+        float lv[kMidKeys];
+#pragma unroll
+        for (int x = 0; x < kMidKeys; ++x) lv[x] = __ldg(lp + min((uint32_t)(tid + kMidThreads * x), N - 1));
+#pragma unroll
+        for (int x = 0; x < kMidKeys; ++x) {
+            const uint32_t idx = (uint32_t)(tid + kMidThreads * x), idc = min(idx, N - 1);
+            const int row = c_shift >= 0 ? (int)(idc >> c_shift) : (int)(idc / (uint32_t)C);
+            const uint32_t o = ord_of(__fadd_rn(sc ? __ldg(sc + row) : 0.f, lv[x]));
+            ords[idx] = o;
+            if (idx < N) { tmax = max(tmax, o); tmin = min(tmin, o); }
+        }
+    }
+    uint32_t mx = tmax, mn = tmin;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+    }
+    if (lane == 0) { sh.wred[0][warp] = mx; sh.wred[1][warp] = mn; }
+    __syncthreads();
+    mx = sh.wred[0][lane]; mn = sh.wred[1][lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+    }
+    const uint32_t span_v = mx - mn;
+    const int nbits = span_v ? 32 - __clz(span_v) : 0;
+    const int sh1 = max(nbits - 11, 0);                            // shift of the top 11-bit digit of (ord - mn)
+
+    // ---- 2. bound from the per-thread maxima ------------------------------------------------------------
+    if ((uint32_t)tid < N) {
+        const uint32_t b = (tmax - mn) >> sh1;
+        atomicAdd(&sh.hist[b], 1u);
+        atomicAdd(&sh.coarse[b >> 5], 1u);
+    }
+    __syncthreads();
+    const uint32_t n_thr = min((uint32_t)kMidThreads, N);          // threads that hold at least one candidate
+    if (warp == 0) {
+        if (K <= n_thr) mid_select(sh, K);
+        else if (lane == 0) sh.sel_bin = 0;
+    }
+    __syncthreads();
+    const uint32_t lb = mn + (sh.sel_bin << sh1);
+
+    auto append = [&](bool f, uint32_t o, uint32_t idx) {
+        const uint32_t bal = __ballot_sync(0xffffffffu, f);
+        if (bal) {
+            const int leader = __ffs(bal) - 1;
+            uint32_t pos = 0;
+            if (lane == leader) pos = atomicAdd(&sh.cursor, (uint32_t)__popc(bal));
+            pos = __shfl_sync(0xffffffffu, pos, leader) + __popc(bal & ((1u << lane) - 1u));
+            if (f && pos < (uint32_t)kMidMaxK) sh.list[pos] = ((unsigned long long)(~o) << 32) | idx;
+        }
+    };
+
+    // ---- 3. survivors ------------------------------------------------------------------------------------
+#pragma unroll 4
+    for (int j = 0; j < kMidKeys; ++j) {
+        const uint32_t idx = (uint32_t)(tid + kMidThreads * j);
+        const uint32_t o = ords[idx];
+        append(idx < N && o >= lb, o, idx);
+    }
+    __syncthreads();
+    uint32_t n_list = sh.cursor;
+    __syncthreads();                                               // (cursor is reset below)
+
+    if (n_list > (uint32_t)kMidMaxK) {
+        // ---- 4. exact selection: value T of the K-th largest (ord - mn), then ties by index ---------------
+        uint32_t pref = 0, rem = K;
+        int shift_prev = 32, width = min(11, nbits), shift = nbits - width;   // first digit: the top `width` bits
+        bool first = true;
+        while (true) {
+            for (int b = tid; b < kBins + kCoarse; b += kMidThreads) sh.hist[b] = 0;
+            __syncthreads();
+#pragma unroll 4
+            for (int j = 0; j < kMidKeys; ++j) {
+                const uint32_t idx = (uint32_t)(tid + kMidThreads * j);
+                const uint32_t v = ords[idx] - mn;
+                if (idx < N && (first || (v >> shift_prev) == pref)) {
+                    const uint32_t dgt = (v >> shift) & ((1u << width) - 1u);
+                    atomicAdd(&sh.hist[dgt], 1u);
+                    atomicAdd(&sh.coarse[dgt >> 5], 1u);
+                }
+            }
+            __syncthreads();
+            if (warp == 0) mid_select(sh, rem);
+            __syncthreads();
+            pref = (pref << width) | sh.sel_bin;
+            rem = sh.sel_rem;
+            first = false;
+            shift_prev = shift;
+            if (shift == 0) break;
+            width = min(11, shift);
+            shift -= width;
+        }
+        const uint32_t T = pref, need = rem;                       // keys > T: K - need; `need` of the keys == T
+        if (tid == 0) sh.cursor = 0;
+        __syncthreads();
+        uint32_t tie_base = 0;
+        for (int j = 0; j < kMidKeys; ++j) {                       // index order: j major, thread minor
+            const uint32_t idx = (uint32_t)(tid + kMidThreads * j);
+            const uint32_t o = ords[idx];
+            const uint32_t v = o - mn;
+            const bool live = idx < N;
+            const bool eq = live && v == T;
+            const uint32_t bal = __ballot_sync(0xffffffffu, eq);
+            if (lane == 0) sh.wred[j & 1][warp] = (uint32_t)__popc(bal);
+            __syncthreads();
+            uint32_t inc = sh.wred[j & 1][lane];                   // inclusive prefix over the warps
+#pragma unroll
+            for (int o2 = 1; o2 < 32; o2 <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o2);
+                if (lane >= o2) inc += t;
+            }
+            const uint32_t before_warp = __shfl_sync(0xffffffffu, inc, warp) - __shfl_sync(0xffffffffu, sh.wred[j & 1][lane], warp);
+            const uint32_t total = __shfl_sync(0xffffffffu, inc, 31);
+            const uint32_t pos = tie_base + before_warp + (uint32_t)__popc(bal & ((1u << lane) - 1u));
+            append((live && v > T) || (eq && pos < need), o, idx);
+            tie_base += total;
+        }
+        __syncthreads();
+        n_list = sh.cursor;                                        // == K
+    }
+
+    // ---- ranking by counting: composites are distinct; ranks < K are the result, in order ---------------
+    n_list = min(n_list, (uint32_t)kMidMaxK);
+    if (tid == 0) { sh.list[n_list] = ~0ull; sh.list[n_list + 1] = ~0ull; }
+    __syncthreads();
+    if ((uint32_t)tid < n_list) {
+        const unsigned long long mine = sh.list[tid];
+        uint32_t rk = 0;
+        const uint32_t n2 = (n_list + 1) & ~1u;
+#pragma unroll 4
+        for (uint32_t i = 0; i < n2; i += 2) {
+            const ulonglong2 c = *reinterpret_cast<const ulonglong2*>(&sh.list[i]);   // broadcast
+            rk += (uint32_t)(c.x < mine) + (uint32_t)(c.y < mine);
+        }
+        if (rk < K) {
+            const uint32_t idx = min((uint32_t)mine, N - 1);
+            const int row = c_shift >= 0 ? (int)(idx >> c_shift) : (int)(idx / (uint32_t)C);
+            const size_t o = (size_t)u * W_out + rk;
+            out_score[o] = __fadd_rn(sc ? __ldg(sc + row) : 0.f, __ldg(lp + idx));
+            out_parent[o] = row;
+            out_code[o] = (int)idx - row * C;
+        }
+    }
+}
+
 int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
 
 }  // namespace
@@ -757,6 +964,20 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
             topk_small_kernel<1><<<B, kSmallThreads, 0, st>>>(logp, score, W_in, C, W_out, out_score, out_parent, out_code);
         else
             topk_small_kernel<2><<<B, kSmallThreads, 0, st>>>(logp, score, W_in, C, W_out, out_score, out_parent, out_code);
+        STARK_LAUNCH_CHECK();
+        return STARK_OK;
+    }
+    if (N <= kMidMaxN && W_out <= kMidMaxK) {
+        static bool mid_attr_done = false;
+        if (!mid_attr_done) {
+            STARK_CUDA_TRY(cudaFuncSetAttribute(topk_mid_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                kMidMaxN * 4));
+            mid_attr_done = true;
+        }
+        int c_sh = -1;
+        if ((C & (C - 1)) == 0) { c_sh = 0; while ((1 << c_sh) < C) ++c_sh; }
+        topk_mid_kernel<<<B, kMidThreads, kMidMaxN * 4, st>>>(logp, score, W_in, C, c_sh, W_out, out_score,
+                                                              out_parent, out_code);
         STARK_LAUNCH_CHECK();
         return STARK_OK;
     }
