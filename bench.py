@@ -496,41 +496,62 @@ def run_stark(args, cfg):
         roof["traffic"] = json.load(open(tpath)).get(cfg.name, {}).get(dom)
 
     # ---- e2e: HOST buffers in, HOST result out, copies inside the timed region ------------------
-    p0, hst = passes[0], hosts[0]
+    # Two device input sets are used in turn (double buffering): the H2D copy of pass i+1 runs on a copy stream
+    # while pass i computes; the host waits for every pass's result (D2H into pinned memory) before it counts it.
     dt_t = torch.float32 if cfg.dtype == "f32" else torch.bfloat16
     pin = lambda a, d=None: (torch.from_numpy(a).to(d) if d is not None else torch.from_numpy(a)).contiguous().pin_memory()
-    src = [pin(hst["K"], dt_t), pin(hst["V"], dt_t), pin(hst["cu"].astype(np.int32))] \
-        + [pin(x, dt_t) for x in hst["q"]] + [pin(x, dt_t) for x in hst["k"]] + [pin(x, dt_t) for x in hst["v"]] \
-        + [x.cpu().pin_memory() for x in p0.logp]
-    dst = [p0.layer.k_prefix, p0.layer.v_prefix, p0.layer.cu] + p0.q + p0.k_new + p0.v_new + p0.logp
-    res_d = [x for s in p0.sel for x in s]
-    res_h = [torch.empty(x.shape, dtype=x.dtype).pin_memory() for x in res_d]
-    h2d = sum(x.numel() * x.element_size() for x in src)
-    d2h = sum(x.numel() * x.element_size() for x in res_h)
+    NB = 2 if R >= 2 else 1
+    bufs = []
+    for bi in range(NB):
+        pb, hst = passes[bi], hosts[bi]
+        src = [pin(hst["K"], dt_t), pin(hst["V"], dt_t), pin(hst["cu"].astype(np.int32))] \
+            + [pin(x, dt_t) for x in hst["q"]] + [pin(x, dt_t) for x in hst["k"]] + [pin(x, dt_t) for x in hst["v"]] \
+            + [x.cpu().pin_memory() for x in pb.logp]
+        dst = [pb.layer.k_prefix, pb.layer.v_prefix, pb.layer.cu] + pb.q + pb.k_new + pb.v_new + pb.logp
+        res_d = [x for s_ in pb.sel for x in s_]
+        res_h = [torch.empty(x.shape, dtype=x.dtype).pin_memory() for x in res_d]
+        bufs.append((src, dst, res_d, res_h))
+    h2d = sum(x.numel() * x.element_size() for x in bufs[0][0])
+    d2h = sum(x.numel() * x.element_size() for x in bufs[0][3])
+    s_in, s_run = torch.cuda.Stream(), torch.cuda.Stream()
+    ev_in = [torch.cuda.Event() for _ in range(NB)]
+    ev_out = [torch.cuda.Event() for _ in range(NB)]
 
-    def e2e_step():
-        for s_, d_ in zip(src, dst):
-            d_.copy_(s_, non_blocking=True)
-        calls[0]()
-        for d_, h_ in zip(res_d, res_h):
-            h_.copy_(d_, non_blocking=True)
-        torch.cuda.current_stream().synchronize()        # the caller reads the result on the host
+    def submit(i):
+        bi = i % NB
+        src, dst, res_d, res_h = bufs[bi]
+        with torch.cuda.stream(s_in):
+            s_in.wait_event(ev_out[bi])                  # the pass that last used this input set has finished
+            for s_, d_ in zip(src, dst):
+                d_.copy_(s_, non_blocking=True)
+            ev_in[bi].record(s_in)
+        with torch.cuda.stream(s_run):
+            s_run.wait_event(ev_in[bi])
+            calls[bi]()
+            for d_, h_ in zip(res_d, res_h):
+                h_.copy_(d_, non_blocking=True)
+            ev_out[bi].record(s_run)
 
-    n_e2e = max(3, min(args.steps, 30))
-    for _ in range(3):
-        e2e_step()
+    def e2e_run(n):
+        submit(0)
+        for i in range(1, n):
+            submit(i)
+            ev_out[(i - 1) % NB].synchronize()           # the caller reads pass i-1's result on the host
+        ev_out[(n - 1) % NB].synchronize()
+
+    n_e2e = max(4, min(args.steps, 40))
+    torch.cuda.synchronize()
+    e2e_run(4)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    e0.record()
-    for _ in range(n_e2e):
-        e2e_step()
-    e1.record()
+    e2e_run(n_e2e)
     torch.cuda.synchronize()
-    e2e_ms = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3) / n_e2e
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / n_e2e
     e2e = {"value": world * sids_per_pass / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": n_e2e,
            "note": "prefix K/V + per-step q/k/v/log-probs copied from pinned host memory every pass; "
-                   "per-level (score,parent,code) read back"}
+                   "per-level (score,parent,code) read back; two input sets in turn, the copy of pass i+1 "
+                   "overlaps pass i (wall clock, host waits for every result)"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
