@@ -314,6 +314,7 @@ def run_reference(args, cfg):
     if rank != 0:
         return
     n_users = 1
+    lens = wl.prefix_lengths(cfg, 0)
     for _ in range(args.warmup):
         pass  # the oracle has no warm-up state; nothing to do
     steps = max(1, min(args.steps, 5))
@@ -328,7 +329,10 @@ def run_reference(args, cfg):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * total / steps * cfg.B / n_users, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg.name, "sample": f"{n_users} of {cfg.B} users per step, all {cfg.d} decode steps"},
+            "config": {"workload": cfg.name, "B": cfg.B, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D,
+                       "prefix_len": [int(lens.min()), int(lens.max())], "beam": list(wl.beam_widths(cfg)),
+                       "levels": cfg.d, "codebook": cfg.C, "decode_steps_per_pass": cfg.d,
+                       "sample": f"{n_users} of {cfg.B} users per step, all {cfg.d} decode steps"},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle",
                              "sample": f"{n_users} of {cfg.B} users x {steps} repeats"},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
