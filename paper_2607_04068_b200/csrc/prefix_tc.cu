@@ -287,7 +287,7 @@ template <int D>
 __device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char* smem_raw, uint32_t ring_off, int ob, int me,
                                           int ns, int lane, uint32_t aO, bool has, float m_own, float l_own,
                                           int u, int n_q, int Hq, int G, int kv, int beam_base, int quarter,
-                                          float* ch_y, const uint32_t* ch_off) {
+                                          float* ch_y, const uint32_t* ch_off, const unsigned char* vstage) {
     constexpr uint32_t SLOT = 32 * D * 4;
     constexpr int CPR = D / 4;                          // 16-byte chunks per fp32 row
     constexpr int CPO = D / 8;                          // 16-byte chunks per bf16 row
@@ -358,8 +358,17 @@ __device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char*
             const uint4* vp0 = reinterpret_cast<const uint4*>(((fa.vn && t0 == level - 1) ? fa.vn : fa.vs) + ch_off[t0]) + c * 4;
             const uint4* vp1 = reinterpret_cast<const uint4*>(((fa.vn && t1 == level - 1) ? fa.vn : fa.vs) + ch_off[t1]) + c * 4;
             uint4 vv[2][4];
+            if (vstage != nullptr && t0 == 0) {         // staged by cp.async right after the last MMA (parity mode)
 #pragma unroll
-            for (int k4 = 0; k4 < 4; ++k4) { vv[0][k4] = __ldg(vp0 + k4); vv[1][k4] = __ldg(vp1 + k4); }
+                for (int k4 = 0; k4 < 4; ++k4) {   // rows of D*2 bytes, 16-byte chunks XOR-swizzled by row
+                    const int ch = ((c * 4 + k4) ^ (lane & 7)) * 16;
+                    vv[0][k4] = *reinterpret_cast<const uint4*>(vstage + (size_t)lane * (D * 2) + ch);
+                    vv[1][k4] = *reinterpret_cast<const uint4*>(vstage + (size_t)((two_lv ? 32 : 0) + lane) * (D * 2) + ch);
+                }
+            } else {
+#pragma unroll
+                for (int k4 = 0; k4 < 4; ++k4) { vv[0][k4] = __ldg(vp0 + k4); vv[1][k4] = __ldg(vp1 + k4); }
+            }
 #pragma unroll
             for (int lv = 0; lv < 2; ++lv)
 #pragma unroll
@@ -531,6 +540,8 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     const int blk = t * 4 + quarter;                    // 32-row block of the CTA's (up to) 256 rows
     const int owner = blk % n_splits, ob = blk / n_splits;                 // cluster rank that finishes it
     const uint32_t me = (FUSED && n_splits > 1) ? cluster_rank() : 0u;
+    // parity mode without splits: only blocks 0..3 finish, ring slots 4..7 are free for the chain's V rows
+    const bool vpre = FUSED && parity && n_splits == 1 && mine && fa.level > 0;
     float ch_y[8];                                      // chain scores, later weights (fused mode)
     uint32_t ch_off[8];                                 // chain row offsets in the suffix buffers
 
@@ -739,6 +750,38 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 mbar_arrive(bar_pfull + 8 * t);
             }
             // ---- epilogue: O row -> partials ----
+            if (FUSED && vpre) {
+                // The V rows of the first two chain levels of this warp's 32 rows go to ring bytes [4, 8) * 32*D*4
+                // (K/V ring tiles 2 and 3; unused by the tail in parity mode without splits) asynchronously, as
+                // soon as the tensor pipe has released those two tiles for the last time -- normally long before
+                // the last MMA, so the copies are issued inside the wait for it and land during the in-CTA merge.
+                // (A trace showed the tail paying one dependent round of V loads per 32-column chunk: 4 x ~1.2 k
+                // cycles.)  The WARP copies row after row, D/8 lanes per row: whole lines per request (lane-per-row
+                // copies cost 32 line slots of the load unit each: 4 k cycles).
+                for (int sl = 2; sl <= 3; ++sl)
+                    if (2 * n_tiles > sl) {
+                        const int n_last = sl + ((2 * n_tiles - 1 - sl) / NS) * NS;   // last tile through this slot
+                        mbar_wait(bar_empty + 8 * sl, (uint32_t)((n_last / NS) & 1));
+                    }
+                constexpr int LPR = D / 8, RPI = 32 / LPR;
+                const int sub = lane % LPR, grp = lane / LPR;
+                const uint32_t live_mask = __ballot_sync(0xffffffffu, live);
+                const uint32_t dst0 = sKV + (uint32_t)(4 + quarter) * (32 * D * 4);
+                const int nlv = min(fa.level, 2);
+                for (int lv = 0; lv < nlv; ++lv) {
+                    const __nv_bfloat16* vbase = (fa.vn && lv == fa.level - 1) ? fa.vn : fa.vs;
+                    const uint32_t my_off = live ? ch_off[lv] : 0u;
+#pragma unroll 4
+                    for (int p = 0; p < 32 / RPI; ++p) {
+                        const int row = p * RPI + grp;
+                        const uint32_t off = __shfl_sync(0xffffffffu, my_off, row);
+                        if ((live_mask >> row) & 1u)
+                            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst0 + (uint32_t)((lv * 32 + row) * (D * 2) + ((sub ^ (row & 7)) * 16))),
+                                         "l"(reinterpret_cast<const uint4*>(vbase + off) + sub) : "memory");
+                    }
+                }
+                asm volatile("cp.async.commit_group;" ::: "memory");
+            }
             if (n_tiles > 0) mbar_wait(bar_done, 0);
             __syncwarp();
             if (parity) {
@@ -855,9 +898,12 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 st_cluster_f2(map_to_rank(ml_base + slot * 256 + (uint32_t)lane * 8, (uint32_t)owner), m_ref, l_sum);
             }
             if (n_splits > 1) cluster_sync_all();                          // B2: all partial rows delivered
-            if (mine && owner == (int)me)
+            if (mine && owner == (int)me) {
+                if (vpre) { asm volatile("cp.async.wait_group 0;" ::: "memory"); __syncwarp(); }
                 fused_finish<D>(fa, smem_raw, sKV - smem_u32(smem_raw), ob, (int)me, n_splits, lane, aO, n_tiles > 0, m_ref,
-                                l_sum, u, n_q, Hq, G, kv, (tile0 + (parity ? 0 : t)) * beams_per_tile, quarter, ch_y, ch_off);
+                                l_sum, u, n_q, Hq, G, kv, (tile0 + (parity ? 0 : t)) * beams_per_tile, quarter, ch_y, ch_off,
+                                vpre ? smem_raw + (sKV - smem_u32(smem_raw)) + (size_t)(4 + quarter) * (32 * D * 4) : nullptr);
+            }
             tc_fence_before();
         }
     }
