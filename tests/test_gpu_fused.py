@@ -76,6 +76,10 @@ def _case(B, Hq, Hkv, D, lens, W, d, seed):
     ("pair_mode_many_ctas", (10, 16, 4, 128, [300] * 10, 70, 2)), # 2 Q tiles per CTA, no splits
     ("gqa1_and_short_prefix", (2, 4, 4, 128, [5, 260], 12, 2)),   # G = 1, a 5-row prefix
     ("gqa8", (2, 16, 2, 128, [640, 384], 16, 2)),                 # G = 8: 16 beams per Q tile
+    # parity mode WITHOUT splits (128 CTAs): chain V rows staged by cp.async into idle ring tiles; 3 levels deep, so
+    # levels 0-1 come from shared memory and level 2 from global memory; ragged prefixes incl. 1- and 2-tile users
+    ("parity_nosplit_d64_deep", (32, 16, 4, 64, [100 + 37 * (x % 14) for x in range(32)], 24, 3)),
+    ("parity_nosplit_d128_deep", (32, 8, 4, 128, [60 + 53 * (x % 11) for x in range(32)], 20, 3)),
 ])
 def test_fused_structural_cases(name, args):
     _case(*args, seed=sum(map(ord, name)))
