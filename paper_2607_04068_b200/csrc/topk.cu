@@ -6,6 +6,12 @@
 //   keep the W_out entries first in (key descending, flat index ascending)
 //   (reading R6), output sorted in that order.
 //
+// Three kernels by problem size (launch_topk): N <= 512 candidates per user: one
+// 256-thread CTA ranking by counting (topk_small_kernel); N <= 16384 and
+// W_out <= 256: one 1024-thread CTA per user, bound from per-thread maxima +
+// ranking by counting (topk_mid_kernel); otherwise the cluster kernel described
+// here (topk_kernel).  All three produce the same total order.
+//
 // The work is tiny next to its latency (1 MB per level at config 2), so the
 // design minimises dependent phases and cross-CTA traffic (measured on B200: a
 // DSMEM pull of whole 8 KB histograms from every rank costs 2-15k cycles, a
