@@ -44,3 +44,34 @@ def select_beams(score: np.ndarray, logp: np.ndarray, W_out: int) -> Tuple[np.nd
     # which compare equal, so the index decides, as IEEE comparison requires.
     order = np.lexsort((idx, -key))[:W_out]
     return key[order].copy(), (order // C).astype(np.int32), (order % C).astype(np.int32)
+
+
+def row_offset_fp32(score: np.ndarray, logits: np.ndarray) -> np.ndarray:
+    """Selection straight from raw logits (reading R22).
+
+    Eq. 1 (PAPER.md:100-103) needs log P(c | ...) = logit_c - logsumexp(logits);
+    the normaliser is one scalar per parent beam, so it is folded into the
+    beam's running score instead of being subtracted from every candidate:
+        lse[i]    = fl32( logsumexp_c logits[i, c] )      (fp64, rounded once)
+        offset[i] = fl32( score[i] - lse[i] )             (one fp32 subtraction)
+    A row whose logits are all -inf (a beam with no legal continuation) has
+    offset = -inf by definition, so that its keys are -inf and never NaN.
+    score[W_in] fp32, logits[W_in, C] fp32 -> offset[W_in] fp32."""
+    score = np.asarray(score, dtype=np.float32)
+    x = np.asarray(logits, dtype=np.float32).astype(np.float64)
+    m = np.max(x, axis=-1)
+    dead = np.isneginf(m)
+    msafe = np.where(dead, 0.0, m)
+    with np.errstate(divide="ignore"):
+        lse = msafe + np.log(np.sum(np.exp(x - msafe[:, None]), axis=-1))
+    lse32 = lse.astype(np.float32)
+    off = (score - lse32).astype(np.float32)
+    return np.where(dead, np.float32(-np.inf), off).astype(np.float32)
+
+
+def select_beams_from_logits(score: np.ndarray, logits: np.ndarray, W_out: int):
+    """Reading R22: key[i*C + c] = fl32(offset[i] + logits[i, c]) with
+    offset = row_offset_fp32(score, logits); then exactly step O4's selection
+    (key descending, flat index ascending).  Same value as score + logp up to
+    the rounding of two fp32 operations."""
+    return select_beams(row_offset_fp32(score, logits), np.asarray(logits, dtype=np.float32), W_out)

@@ -127,3 +127,67 @@ def test_log_softmax_pins():
     # probabilities sum to one; huge logits do not overflow
     big = log_softmax_fp32(np.array([[1e4, 1e4 - 1.0, -1e4]]))
     assert np.all(np.isfinite(big)) and abs(np.exp(big.astype(np.float64)).sum() - 1) < 1e-6
+
+
+# ---- selection from raw logits (reading R22) ---------------------------------------------------------------
+
+def test_row_offset_matches_library_logsumexp_and_closed_forms():
+    from scipy.special import logsumexp
+    from oracle.selection import row_offset_fp32
+    rng = np.random.default_rng(5)
+    logits = (rng.standard_normal((37, 301)) * 2).astype(np.float32)
+    score = rng.standard_normal(37).astype(np.float32)
+    off = row_offset_fp32(score, logits)
+    ref = (score - logsumexp(logits.astype(np.float64), axis=-1).astype(np.float32)).astype(np.float32)
+    assert off.dtype == np.float32 and np.array_equal(off, ref)
+    # closed form: C equal logits a  =>  lse = a + ln C
+    for C in (1, 2, 8, 1000):
+        a = np.float32(1.75)
+        o = row_offset_fp32(np.zeros(1, np.float32), np.full((1, C), a, np.float32))
+        assert o[0] == np.float32(-np.float32(float(a) + math.log(C)))
+    # one dominant logit: lse -> that logit
+    big = np.full((1, 64), -200.0, np.float32); big[0, 17] = 3.0
+    assert row_offset_fp32(np.float32([0.5]), big)[0] == np.float32(0.5 - 3.0)
+    # huge logits do not overflow (max subtraction); dead rows give -inf, not NaN
+    assert row_offset_fp32(np.float32([0.0]), np.full((1, 4), 1e30, np.float32))[0] == np.float32(-1e30)
+    dead = row_offset_fp32(np.float32([0.0, 1.0]), np.float32([[-np.inf] * 3, [0.0, -np.inf, -np.inf]]))
+    assert np.isneginf(dead[0]) and dead[1] == np.float32(1.0)
+
+
+def test_select_from_logits_agrees_with_logprob_selection():
+    """The folded key differs from fl32(score + logp) by at most a few ulp, so: the keys agree to
+    4 ulp-of-magnitude, probabilities of a row still sum to 1, and on inputs with wide margins
+    (logits on a coarse grid of distinct values) the selected (parent, code) lists are identical."""
+    from oracle.selection import select_beams_from_logits, row_offset_fp32
+    rng = np.random.default_rng(11)
+    W_in, C, W_out = 12, 40, 30
+    logits = rng.permutation(W_in * C).reshape(W_in, C).astype(np.float32) * np.float32(0.03125) - 7
+    score = -rng.random(W_in).astype(np.float32)
+    s1, p1, c1 = select_beams_from_logits(score, logits, W_out)
+    s0, p0, c0 = select_beams(score, log_softmax_fp32(logits), W_out)
+    assert np.array_equal(p1, p0) and np.array_equal(c1, c0)
+    assert np.max(np.abs(s1.astype(np.float64) - s0)) <= 4 * np.spacing(np.float32(np.max(np.abs(s0))))
+    off = row_offset_fp32(np.zeros(W_in, np.float32), logits)
+    total = np.exp((off[:, None] + logits).astype(np.float64)).sum(axis=-1)
+    assert np.allclose(total, 1.0, atol=1e-5)
+
+
+def test_select_from_logits_shift_invariance_and_ties():
+    """Adding a power-of-two-exact constant to every logit of a row changes nothing that is selected
+    when all quantities stay exactly representable; exact ties go to the lower flat index."""
+    from oracle.selection import select_beams_from_logits
+    logits = np.float32([[0.0, 0.0, -1.0, 0.0], [0.0, -1.0, 0.0, 0.0]])
+    score = np.float32([0.0, 0.0])
+    s, p, c = select_beams_from_logits(score, logits, 5)
+    # both rows have the same multiset of logits => same lse => keys tie across rows; index order decides
+    assert list(zip(p.tolist(), c.tolist())) == [(0, 0), (0, 1), (0, 3), (1, 0), (1, 2)]
+    assert np.all(s == s[0])
+    shifted = logits + np.float32([[8.0], [-16.0]])
+    s2, p2, c2 = select_beams_from_logits(score, shifted, 5)
+    assert np.array_equal(p2, p) and np.array_equal(c2, c)
+    assert np.allclose(s2, s, atol=1e-6)
+    # a dead row (all -inf) sorts last and yields -inf keys, never NaN
+    lg = np.float32([[-np.inf, -np.inf], [0.0, 1.0]])
+    s3, p3, c3 = select_beams_from_logits(np.float32([5.0, 0.0]), lg, 4)
+    assert p3.tolist() == [1, 1, 0, 0] and c3.tolist() == [1, 0, 0, 1]
+    assert not np.any(np.isnan(s3)) and np.all(np.isneginf(s3[2:]))
