@@ -80,7 +80,8 @@ typedef enum stark_call {
     STARK_CALL_PREFIX_ATTN = 0,
     STARK_CALL_TREE_ATTN_STEP = 1,
     STARK_CALL_BEAM_TOPK = 2,
-    STARK_CALL_KV_APPEND_REORG = 3
+    STARK_CALL_KV_APPEND_REORG = 3,
+    STARK_CALL_BEAM_TOPK_LOGITS = 4
 } stark_call_t;
 
 /* Static shape of one attention layer's decode problem. */
@@ -246,6 +247,33 @@ int stark_decode_step(const stark_shape_t* shape, const void* q, int n_q, int le
 int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_in, int C,
                     int W_out, float* out_score, int32_t* out_parent, int32_t* out_code,
                     void* ws, size_t ws_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------
+ * A3'. Beam selection straight from raw logits  (
+ *      DESIGN.md reading R22)
+ *
+ * Eq. 1 needs log P(c | ...) = logit_c - logsumexp(logits of
+ * the parent beam).  The normaliser is one scalar per parent beam; it is folded
+ * into the beam's running score, the candidates are never rewritten:
+ *     lse[u,i]    = fl32( logsumexp_c logits[u,i,c] )   fp64 arithmetic, rounded once
+ *     offset[u,i] = fl32( score[u,i] - lse[u,i] )       ONE fp32 subtraction;
+ *                   -inf if every logit of the beam is -inf (no legal continuation)
+ *     key[i*C + c] = fl32( offset[u,i] + logits[u,i,c] ) ONE fp32 addition
+ * followed by exactly stark_beam_topk's selection and outputs (out_score = key,
+ * the new cumulative log-probability).  Equal to score + log-softmax(logits) up
+ * to the rounding of the two fp32 operations; +inf logits are undefined.
+ *
+ * stark_logits_row_offset is the first half on its own (rows = B*W_in beams,
+ * logits [rows, C] fp32, score [rows] fp32 or NULL => zeros, offset out [rows]).
+ * stark_beam_topk_logits runs both; ws, ws_bytes = workspace of
+ * stark_workspace_bytes(shape (B only), STARK_CALL_BEAM_TOPK_LOGITS, W_in, C).
+ * Errors: as stark_beam_topk; the workspace is always required.
+ */
+int stark_logits_row_offset(const float* logits, const float* score_or_null, int64_t rows, int C,
+                            float* offset, void* stream);
+int stark_beam_topk_logits(const float* logits, const float* score_or_null, int B, int W_in, int C,
+                           int W_out, float* out_score, int32_t* out_parent, int32_t* out_code,
+                           void* ws, size_t ws_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------
  * A4. KV append + index reorganisation

@@ -6,6 +6,7 @@
 from .binding import (  # noqa: F401
     StarkError, Shape, make_shape, lib, LIB_PATH, EXPORTS,
     stark_prefix_attn, stark_prefix_attn_plan, stark_tree_attn_step, stark_decode_attn, stark_beam_topk,
+    stark_logits_row_offset, stark_beam_topk_logits,
     stark_kv_append_reorg, stark_workspace_bytes, alloc_partials, alloc_suffix,
-    CALL_PREFIX_ATTN, CALL_TREE_ATTN_STEP, CALL_BEAM_TOPK, CALL_KV_APPEND_REORG,
+    CALL_PREFIX_ATTN, CALL_TREE_ATTN_STEP, CALL_BEAM_TOPK, CALL_KV_APPEND_REORG, CALL_BEAM_TOPK_LOGITS,
 )

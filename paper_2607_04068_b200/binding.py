@@ -8,7 +8,7 @@ from __future__ import annotations
 
 import ctypes
 import os
-from ctypes import POINTER, Structure, byref, c_float, c_int, c_int32, c_size_t, c_void_p
+from ctypes import POINTER, Structure, byref, c_float, c_int, c_int32, c_int64, c_size_t, c_void_p
 from typing import Optional, Tuple
 
 import torch
@@ -17,10 +17,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libstark.so")
 
 STARK_F32, STARK_BF16 = 0, 1
-CALL_PREFIX_ATTN, CALL_TREE_ATTN_STEP, CALL_BEAM_TOPK, CALL_KV_APPEND_REORG = 0, 1, 2, 3
+CALL_PREFIX_ATTN, CALL_TREE_ATTN_STEP, CALL_BEAM_TOPK, CALL_KV_APPEND_REORG, CALL_BEAM_TOPK_LOGITS = 0, 1, 2, 3, 4
 EXPORTS = (
     "stark_prefix_attn", "stark_prefix_attn_plan", "stark_tree_attn_step", "stark_decode_attn", "stark_decode_step",
-    "stark_beam_topk",
+    "stark_beam_topk", "stark_logits_row_offset", "stark_beam_topk_logits",
     "stark_kv_append_reorg", "stark_workspace_bytes", "stark_suffix_bytes",
     "stark_anc_bytes", "stark_version", "stark_status_string", "stark_last_cuda_error",
     "stark_calib_empty", "stark_calib_stream_read",
@@ -72,6 +72,10 @@ def lib() -> ctypes.CDLL:
     L.stark_beam_topk.restype = c_int
     L.stark_beam_topk.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p,
                                   c_void_p, c_size_t, c_void_p]
+    L.stark_logits_row_offset.restype = c_int
+    L.stark_logits_row_offset.argtypes = [c_void_p, c_void_p, c_int64, c_int, c_void_p, c_void_p]
+    L.stark_beam_topk_logits.restype = c_int
+    L.stark_beam_topk_logits.argtypes = L.stark_beam_topk.argtypes
     L.stark_kv_append_reorg.restype = c_int
     L.stark_kv_append_reorg.argtypes = [P, c_int, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
                                         c_void_p, c_void_p]
@@ -176,6 +180,23 @@ def stark_beam_topk(logp: torch.Tensor, score: Optional[torch.Tensor], B: int, W
     _check(lib().stark_beam_topk(_ptr(logp), _ptr(score), B, W_in, C, W_out, _ptr(out_score), _ptr(out_parent),
                                  _ptr(out_code), _ptr(ws), ws.numel() * ws.element_size() if ws is not None else 0,
                                  _stream()), "stark_beam_topk")
+
+
+def stark_logits_row_offset(logits: torch.Tensor, score: Optional[torch.Tensor], rows: int, C: int,
+                            offset: torch.Tensor) -> None:
+    """A3' first half: offset = fl32(score - fl32(logsumexp(logits))) per beam (reading R22)."""
+    _check(lib().stark_logits_row_offset(_ptr(logits), _ptr(score), rows, C, _ptr(offset), _stream()),
+           "stark_logits_row_offset")
+
+
+def stark_beam_topk_logits(logits: torch.Tensor, score: Optional[torch.Tensor], B: int, W_in: int, C: int,
+                           W_out: int, out_score: torch.Tensor, out_parent: torch.Tensor, out_code: torch.Tensor,
+                           ws: Optional[torch.Tensor] = None) -> None:
+    """A3': beam selection straight from raw logits (log-softmax normaliser folded into the beam score)."""
+    _check(lib().stark_beam_topk_logits(_ptr(logits), _ptr(score), B, W_in, C, W_out, _ptr(out_score),
+                                        _ptr(out_parent), _ptr(out_code), _ptr(ws),
+                                        ws.numel() * ws.element_size() if ws is not None else 0, _stream()),
+           "stark_beam_topk_logits")
 
 
 def stark_kv_append_reorg(shape: Shape, level: int, n_new: int, k_new: torch.Tensor, v_new: torch.Tensor,

@@ -19,7 +19,7 @@ INCLUDE = os.path.join(ROOT, "include")
 LIB_PATH = os.path.join(HERE, "libstark.so")
 OBJ_DIR = os.path.join(HERE, "build")
 
-SOURCES = ["api.cu", "append.cu", "tree_attn.cu", "prefix_simt.cu", "prefix_tc.cu", "topk.cu"]
+SOURCES = ["api.cu", "append.cu", "tree_attn.cu", "prefix_simt.cu", "prefix_tc.cu", "topk.cu", "logits_offset.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC]
 

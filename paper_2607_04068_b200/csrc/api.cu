@@ -61,6 +61,9 @@ int check_device() {
     return ok == -2 ? STARK_ERR_CUDA : STARK_ERR_UNSUPPORTED;
 }
 
+// Per-beam offsets of stark_beam_topk_logits, at the front of its workspace (256-byte multiple).
+size_t offset_bytes(int B, int W_in) { return (((size_t)B * W_in * sizeof(float)) + 255) / 256 * 256; }
+
 int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 // Shape-only split choice.  Cost model: waves of CTAs x (KV tiles per CTA + a
@@ -151,6 +154,10 @@ size_t stark_workspace_bytes(const stark_shape_t* s, int call, int n_q, int tota
     if (call == STARK_CALL_BEAM_TOPK) {
         if (s->B < 1 || n_q < 1 || total_tokens < 1) return 0;
         return topk_workspace_bytes(s->B, n_q, total_tokens);
+    }
+    if (call == STARK_CALL_BEAM_TOPK_LOGITS) {
+        if (s->B < 1 || n_q < 1 || total_tokens < 1) return 0;
+        return offset_bytes(s->B, n_q) + topk_workspace_bytes(s->B, n_q, total_tokens);
     }
     return 0;
 }
@@ -271,6 +278,32 @@ int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_
     if (rc != STARK_OK) return rc;
     return launch_topk(logp, score_or_null, B, W_in, C, W_out, out_score, out_parent, out_code, ws, ws_bytes,
                        (cudaStream_t)stream);
+}
+
+int stark_logits_row_offset(const float* logits, const float* score_or_null, int64_t rows, int C,
+                            float* offset, void* stream) {
+    if (!logits || !offset || rows < 1 || C < 1) return STARK_ERR_INVALID_ARG;
+    const int rc = check_device();
+    if (rc != STARK_OK) return rc;
+    return launch_row_offset(logits, score_or_null, (long long)rows, C, offset, (cudaStream_t)stream);
+}
+
+int stark_beam_topk_logits(const float* logits, const float* score_or_null, int B, int W_in, int C, int W_out,
+                           float* out_score, int32_t* out_parent, int32_t* out_code, void* ws,
+                           size_t ws_bytes, void* stream) {
+    if (!logits || !out_score || !out_parent || !out_code) return STARK_ERR_INVALID_ARG;
+    if (B < 1 || W_in < 1 || C < 1 || W_out < 1) return STARK_ERR_INVALID_ARG;
+    if ((long long)W_in * C >= (1ll << 31)) return STARK_ERR_INVALID_ARG;
+    if ((long long)W_out > (long long)W_in * C || W_out > 4096) return STARK_ERR_INVALID_ARG;
+    const size_t off_bytes = offset_bytes(B, W_in), tk_bytes = topk_workspace_bytes(B, W_in, C);
+    if (!ws || ws_bytes < off_bytes + tk_bytes) return STARK_ERR_WORKSPACE;
+    int rc = check_device();
+    if (rc != STARK_OK) return rc;
+    float* offset = static_cast<float*>(ws);
+    rc = launch_row_offset(logits, score_or_null, (long long)B * W_in, C, offset, (cudaStream_t)stream);
+    if (rc != STARK_OK) return rc;
+    return launch_topk(logits, offset, B, W_in, C, W_out, out_score, out_parent, out_code,
+                       static_cast<char*>(ws) + off_bytes, ws_bytes - off_bytes, (cudaStream_t)stream);
 }
 
 int stark_kv_append_reorg(const stark_shape_t* shape, int level, int n_new, const void* k_new,

@@ -109,6 +109,8 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
                 float* out_score, int32_t* out_parent, int32_t* out_code, void* ws, size_t ws_bytes,
                 cudaStream_t st);
 size_t topk_workspace_bytes(int B, int W_in, int C);
+int launch_row_offset(const float* logits, const float* score, long long rows, int C, float* offset,
+                      cudaStream_t st);
 int launch_calib(const void* src_or_null, size_t bytes, void* sink, cudaStream_t st);
 
 }  // namespace stark

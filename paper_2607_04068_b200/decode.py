@@ -102,3 +102,21 @@ def beam_topk(logp: torch.Tensor, score: Optional[torch.Tensor], W_out: int,
                torch.empty((B, W_out), dtype=torch.int32, device=logp.device))
     sb.stark_beam_topk(logp, score, B, W_in, C, W_out, out[0], out[1], out[2])
     return out
+
+
+def beam_topk_logits(logits: torch.Tensor, score: Optional[torch.Tensor], W_out: int,
+                     out: Optional[Tuple[torch.Tensor, torch.Tensor, torch.Tensor]] = None,
+                     ws: Optional[torch.Tensor] = None):
+    """logits[B,W_in,C] fp32 (raw), score[B,W_in] fp32 or None -> (score, parent, code) [B,W_out]
+    (include/stark.h A3': the log-softmax normaliser is folded into the beam score)."""
+    B, W_in, C = logits.shape
+    if out is None:
+        out = (torch.empty((B, W_out), dtype=torch.float32, device=logits.device),
+               torch.empty((B, W_out), dtype=torch.int32, device=logits.device),
+               torch.empty((B, W_out), dtype=torch.int32, device=logits.device))
+    if ws is None:
+        shape = sb.make_shape(B=B, Hq=1, Hkv=1, D=64, d=1, Wmax=W_in, dtype=torch.float32)
+        ws = torch.empty(sb.stark_workspace_bytes(shape, sb.CALL_BEAM_TOPK_LOGITS, W_in, C), dtype=torch.uint8,
+                         device=logits.device)
+    sb.stark_beam_topk_logits(logits, score, B, W_in, C, W_out, out[0], out[1], out[2], ws)
+    return out
