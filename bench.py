@@ -41,6 +41,8 @@ def parse_args():
     ap.add_argument("--impl", default="stark", choices=["stark", "reference"])
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--from-logits", action="store_true",
+                    help="selection consumes RAW logits (stark_beam_topk_logits, SURVEY 8f-1) instead of log-probs")
     ap.add_argument("--no-graph", action="store_true", help="launch eagerly instead of replaying CUDA graphs")
     ap.add_argument("--sets", type=int, default=0, help="rotating input sets (0 = enough to exceed L2)")
     ap.add_argument("--calibrate", action="store_true",
@@ -102,17 +104,18 @@ def host_inputs(cfg, seed):
     return dict(K=K, V=V, cu=cu, q=q, k=k, v=v, lg=lg)
 
 
-def make_pass(cfg, h, dev):
+def make_pass(cfg, h, dev, from_logits=False):
     import torch
     from paper_2607_04068_b200.pipeline import DecodePass
     dt = torch.float32 if cfg.dtype == "f32" else torch.bfloat16
     up = lambda a, d=None: (torch.from_numpy(a).to(dev).to(d) if d is not None else torch.from_numpy(a).to(dev)).contiguous()
     # log-softmax of the per-level logits is the caller's step before stark_beam_topk: untimed
-    logp = [torch.log_softmax(up(x), dim=-1).contiguous() for x in h["lg"]]
+    # (--from-logits: the raw logits go to stark_beam_topk_logits, the normalisation is inside the timed pass)
+    logp = [up(x) if from_logits else torch.log_softmax(up(x), dim=-1).contiguous() for x in h["lg"]]
     lens = np.diff(h["cu"])
     return DecodePass(cfg.B, cfg.Hq, cfg.Hkv, cfg.D, cfg.d, cfg.C, wl.beam_widths(cfg), dt, up(h["K"], dt),
                       up(h["V"], dt), up(h["cu"].astype(np.int32)), int(lens.max()), [up(x, dt) for x in h["q"]],
-                      [up(x, dt) for x in h["k"]], [up(x, dt) for x in h["v"]], logp)
+                      [up(x, dt) for x in h["k"]], [up(x, dt) for x in h["v"]], logp, from_logits=from_logits)
 
 
 class ClockSampler(threading.Thread):
@@ -368,7 +371,7 @@ def run_stark(args, cfg):
         + sum(a.nbytes for a in h0["lg"])
     R = args.sets or int(min(16, max(2, -(-2 * L2_BYTES // set_bytes))))
     hosts = [h0] + [host_inputs(cfg, seed=shard_seed(rank, r)) for r in range(1, R)]
-    passes = [make_pass(cfg, h, dev) for h in hosts]
+    passes = [make_pass(cfg, h, dev, from_logits=args.from_logits) for h in hosts]
     lens = np.diff(h0["cu"])
     widths = wl.beam_widths(cfg)
     nq = wl.queries_per_step(cfg)
@@ -471,9 +474,10 @@ def run_stark(args, cfg):
             us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.tree(t, p.q[t], p.out[t])) for p in passes], it, use_graph)
             kern[f"tree_attn_step.t{t}"] = {"us": us, "bytes": work_tree(cfg, nq[t], t, ns)}
         w_in = nq[t]
-        us = time_graph_loop(torch, [(lambda p=p, t=t: beam_topk(p.logp[t], p.sel[t - 1][0] if t else None, widths[t],
-                                                                  out=p.sel[t])) for p in passes], it, use_graph)
-        kern[f"beam_topk.t{t}"] = {"us": us, "bytes": work_topk(cfg, w_in, widths[t])}
+        us = time_graph_loop(torch, [(lambda p=p, t=t: p.select(t, p.sel[t - 1][0] if t else None))
+                                     for p in passes], it, use_graph)
+        kern[("beam_topk_logits" if args.from_logits else "beam_topk") + f".t{t}"] = {
+            "us": us, "bytes": work_topk(cfg, w_in, widths[t])}
         if t >= 1 and not passes[0].inline_append:
             us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.append(t, p.k_new[t], p.v_new[t], p.sel[t - 1][1]))
                                          for p in passes], it, use_graph)
@@ -563,6 +567,7 @@ def run_stark(args, cfg):
             "config": {"workload": cfg.name, "B": cfg.B, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D,
                        "prefix_len": [int(lens.min()), int(lens.max())], "beam": list(widths), "levels": cfg.d,
                        "codebook": cfg.C, "decode_steps_per_pass": cfg.d,
+                       "selection": "raw logits (stark_beam_topk_logits)" if args.from_logits else "log-probs",
                        "l2": f"{R} rotating input sets ({R * set_bytes / 2**20:.0f} MiB > L2 126 MiB), no flush",
                        "launch": f"cuda_graph ({R} passes, one per input set, per graph)" if use_graph else "eager"},
             "us_per_decode_step": ms_per_step * 1e3 / cfg.d,

@@ -14,14 +14,15 @@ from typing import Dict, List, Optional
 
 import torch
 
-from .decode import StarkLayer, beam_topk
+from . import binding as sb
+from .decode import StarkLayer, beam_topk, beam_topk_logits
 
 
 class DecodePass:
     def __init__(self, B: int, Hq: int, Hkv: int, D: int, d: int, C: int, widths: List[int], dtype: torch.dtype,
                  k_prefix: torch.Tensor, v_prefix: torch.Tensor, cu_seqlens: torch.Tensor, max_prefix_len: int,
                  q: List[torch.Tensor], k_new: List[torch.Tensor], v_new: List[torch.Tensor],
-                 logp: List[torch.Tensor], inline_append: bool = True):
+                 logp: List[torch.Tensor], inline_append: bool = True, from_logits: bool = False):
         self.B, self.d, self.C, self.widths = B, d, C, list(widths)
         self.n_q = [1] + self.widths                      # queries per user at step t
         self.fused = dtype == torch.bfloat16 and int(k_prefix.shape[0]) > 0
@@ -30,6 +31,14 @@ class DecodePass:
                                 max_prefix_len, n_q_per_step=None if self.fused else self.n_q[:d])
         self.q, self.k_new, self.v_new, self.logp = q, k_new, v_new, logp
         dev = k_prefix.device
+        # from_logits: `logp` holds RAW per-level logits and the selection is stark_beam_topk_logits (A3':
+        # the log-softmax normaliser is folded into the beam score, two launches per level)
+        self.from_logits = from_logits
+        self.topk_ws = None
+        if from_logits:
+            shp = sb.make_shape(B, 1, 1, 64, 1, max(self.n_q), torch.float32)
+            need = max(sb.stark_workspace_bytes(shp, sb.CALL_BEAM_TOPK_LOGITS, self.n_q[t], C) for t in range(d))
+            self.topk_ws = torch.empty(need, dtype=torch.uint8, device=dev)
         self.out = [torch.empty_like(q[t]) for t in range(d)]
         self.sel = [(torch.empty((B, w), dtype=torch.float32, device=dev),
                      torch.empty((B, w), dtype=torch.int32, device=dev),
@@ -39,7 +48,8 @@ class DecodePass:
     #: unless it rides inside the attention launch
     @property
     def launches(self) -> int:
-        return (2 if self.fused else 3) * self.d + (0 if self.inline_append else self.d - 1)
+        return ((2 if self.fused else 3) * self.d + (0 if self.inline_append else self.d - 1)
+                + (self.d if self.from_logits else 0))
 
     def run(self) -> None:
         score = parent = None
@@ -51,7 +61,12 @@ class DecodePass:
                 if t >= 1:
                     self.layer.append(t, self.k_new[t], self.v_new[t], parent)
                 self.layer.attend(t, self.q[t], out=self.out[t], fused=self.fused)
-            score, parent, _ = beam_topk(self.logp[t], score, self.widths[t], out=self.sel[t])
+            score, parent, _ = self.select(t, score)
+
+    def select(self, t: int, score: Optional[torch.Tensor]):
+        if self.from_logits:
+            return beam_topk_logits(self.logp[t], score, self.widths[t], out=self.sel[t], ws=self.topk_ws)
+        return beam_topk(self.logp[t], score, self.widths[t], out=self.sel[t])
 
     def result(self) -> Dict[str, List[torch.Tensor]]:
         return {"score": [s[0] for s in self.sel], "parent": [s[1] for s in self.sel],

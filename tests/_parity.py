@@ -121,18 +121,19 @@ def run_teacher_forced(cfg, seed=0, final_step=True):
 
 
 # ---- full-size configs: the launch configuration bench.py times, sampled oracle checks -------------
-def run_full_size(cfg, n_samples=6, seed=0, use_graph=True):
+def run_full_size(cfg, n_samples=6, seed=0, use_graph=True, from_logits=False):
     """Free-running DecodePass (bench.py's own object, CUDA-graph replay) at BASELINE.json's full size.
     Checks: (a) every level's selection, ALL users, bit-exact vs oracle.select_beams on the identical fp32
     log-probs and scores; (b) the ancestor index vs oracle.ancestor_chains and the suffix K/V (bitwise copy);
     (c) attention rows of sampled (user, beam) pairs vs oracle.replay_beam_attention (conventional
     per-beam full-sequence attention, fp64); (d) the prefix buffers are bit-identical before/after."""
     import bench
-    from oracle.selection import select_beams
+    from oracle.selection import select_beams, select_beams_from_logits
     from oracle.tree import ancestor_chains
     from oracle.replay import replay_beam_attention
     h = bench.host_inputs(cfg, seed)
-    p = bench.make_pass(cfg, h, torch.device("cuda"))
+    p = bench.make_pass(cfg, h, torch.device("cuda"), from_logits=from_logits)
+    oracle_select = select_beams_from_logits if from_logits else select_beams   # p.logp holds raw logits then
     kp0, vp0 = p.layer.k_prefix.clone(), p.layer.v_prefix.clone()
     p.run()
     torch.cuda.synchronize()
@@ -159,7 +160,7 @@ def run_full_size(cfg, n_samples=6, seed=0, use_graph=True):
         ok = True
         for u in range(cfg.B):
             score = np.zeros(1, np.float32) if t == 0 else sel[t - 1][0][u]
-            s_r, p_r, c_r = select_beams(score, logp[t][u], p.widths[t])
+            s_r, p_r, c_r = oracle_select(score, logp[t][u], p.widths[t])
             ok &= (np.array_equal(sel[t][1][u], p_r) and np.array_equal(sel[t][2][u], c_r)
                    and np.array_equal(sel[t][0][u].view(np.uint32), s_r.view(np.uint32)))
         report.append(("topk_all_users", t, bool(ok), f"N={logp[t].shape[1] * cfg.C} W_out={p.widths[t]}"))

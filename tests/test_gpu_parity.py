@@ -28,3 +28,14 @@ def test_full_size_parity(name):
     rep = run_full_size(wl.get_config(name))
     bad = [r for r in rep if not r[2]]
     assert not bad, f"{name}: {bad}\nfull report: {rep}"
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg4"])
+def test_full_size_parity_from_logits(name):
+    """The same pass with the selection fed RAW logits (stark_beam_topk_logits, reading R22; bench.py
+    --from-logits): every level's (score, parent, code) bit-exact vs oracle.select_beams_from_logits, the
+    tree that results still appended and attended correctly."""
+    from _parity import run_full_size
+    rep = run_full_size(wl.get_config(name), n_samples=3, from_logits=True)
+    bad = [r for r in rep if not r[2]]
+    assert not bad, f"{name}: {bad}\nfull report: {rep}"
