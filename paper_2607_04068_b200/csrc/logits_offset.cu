@@ -12,8 +12,10 @@
 //
 // HBM-bound stream: 4 B per candidate read once; the row stays in registers between the max pass and the
 // sum pass (up to 32 floats per thread; longer rows re-read their tail through L1/L2).  A warp per row for
-// C <= 1024, a 256-thread CTA per row above.  The exponentials are fp64 so that the fp32 result is the
-// correctly rounded one the oracle defines (a different summation order moves the fp64 sum by ~1e-16).
+// C <= 1024, a 256-thread CTA per row above.  The exponentials are fp64 (exp_neg below) so that the fp32
+// result is the correctly rounded one the oracle defines (a different summation order or a last-bit
+// difference of exp moves the fp64 sum by ~1e-16 relative: a flipped fp32 rounding needs the exact value
+// within ~1e-9 ulp of a rounding boundary).
 #include <math.h>
 
 #include "common.cuh"
@@ -24,6 +26,30 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr int kRegVec = 8;  // float4 per thread kept between the two passes
+
+// exp(d) for d <= 0 in fp64, error < 1 ulp + the table's: d = (64 e + j) ln2/64 + r, |r| <= ln2/128,
+// exp(d) = 2^e * 2^(j/64) * exp(r).  exp(r) is the degree-5 Taylor polynomial (remainder r^6/720 < 3.6e-17);
+// 2^(j/64) comes from a 64-entry shared-memory table (filled with exp2() by each CTA); 2^e is an exponent
+// add.  13 fp64 operations against ~25 of the library exp(): the kernel is fp64-pipe-bound at large C.
+// Terms below e^-700 (they cannot move a sum that is >= 1) return 0, which also covers d = -inf.
+__device__ __forceinline__ double exp_neg(double d, const double* __restrict__ tab) {
+    if (d < -700.0) return 0.0;
+    const double kMagic = 6755399441055744.0;                 // 2^52 + 2^51: round-to-nearest-integer by addition
+    const double t = fma(d, 92.332482616893656, kMagic);      // d * 64/ln2
+    const int k = __double2loint(t);                          // integer in the low word (two's complement)
+    const double kf = t - kMagic;
+    // r = d - k ln2/64 in two steps: the high part has 32 significant bits, so kf * hi is exact for |k| < 2^20
+    double r = fma(kf, -0.01083042469326756, d);
+    r = fma(kf, -2.9815858269852933e-12, r);
+    double p = fma(r, 1.0 / 120.0, 1.0 / 24.0);
+    p = fma(p, r, 1.0 / 6.0);
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    p = fma(p, r, 1.0);
+    const double v = tab[k & 63] * p;                          // in (0.99, 2.01)
+    const int e = k >> 6;                                      // floor(k / 64) >= -1010: the result stays normal
+    return __hiloint2double(__double2hiint(v) + (e << 20), __double2loint(v));
+}
 
 __device__ __forceinline__ float max4(float4 v) { return fmaxf(fmaxf(v.x, v.y), fmaxf(v.z, v.w)); }
 
@@ -66,6 +92,9 @@ row_offset_kernel(const float* __restrict__ logits, const float* __restrict__ sc
     constexpr int kRows = kThreads / kTPR;  // rows per CTA and iteration
     __shared__ float sm[kThreads / 32];
     __shared__ double sd[kThreads / 32];
+    __shared__ double tab[64];  // 2^(j/64)
+    if (threadIdx.x < 64) tab[threadIdx.x] = exp2((double)threadIdx.x * (1.0 / 64.0));
+    __syncthreads();
     const int t = threadIdx.x % kTPR, r_in = threadIdx.x / kTPR;
     const float ninf = __int_as_float(0xff800000);
 
@@ -95,14 +124,14 @@ row_offset_kernel(const float* __restrict__ logits, const float* __restrict__ sc
 #pragma unroll
                 for (int x = 0; x < kRegVec; ++x) {
                     if (x * kTPR + t < C4) {
-                        s += exp((double)v[x].x - md); s += exp((double)v[x].y - md);
-                        s += exp((double)v[x].z - md); s += exp((double)v[x].w - md);
+                        s += exp_neg((double)v[x].x - md, tab); s += exp_neg((double)v[x].y - md, tab);
+                        s += exp_neg((double)v[x].z - md, tab); s += exp_neg((double)v[x].w - md, tab);
                     }
                 }
                 for (int j = kRegVec * kTPR + t; j < C4; j += kTPR) {
                     const float4 w = __ldg(p4 + j);
-                    s += exp((double)w.x - md); s += exp((double)w.y - md);
-                    s += exp((double)w.z - md); s += exp((double)w.w - md);
+                    s += exp_neg((double)w.x - md, tab); s += exp_neg((double)w.y - md, tab);
+                    s += exp_neg((double)w.z - md, tab); s += exp_neg((double)w.w - md, tab);
                 }
             }
         } else {
@@ -111,7 +140,7 @@ row_offset_kernel(const float* __restrict__ logits, const float* __restrict__ sc
             m = row_max<kTPR>(m, sm);
             if (m != ninf) {
                 const double md = (double)m;
-                for (int j = t; j < C; j += kTPR) s += exp((double)__ldg(p + j) - md);
+                for (int j = t; j < C; j += kTPR) s += exp_neg((double)__ldg(p + j) - md, tab);
             }
         }
         s = row_sum<kTPR>(s, sd);
