@@ -31,18 +31,25 @@ constexpr int kRegVec = 8;  // float4 per thread kept between the two passes
 // exp(d) = 2^e * 2^(j/64) * exp(r).  exp(r) is the degree-5 Taylor polynomial (remainder r^6/720 < 3.6e-17);
 // 2^(j/64) comes from a 64-entry shared-memory table (filled with exp2() by each CTA); 2^e is an exponent
 // add.  13 fp64 operations against ~25 of the library exp(): the kernel is fp64-pipe-bound at large C.
-// Terms below e^-700 (they cannot move a sum that is >= 1) return 0, which also covers d = -inf.
+// The caller clamps the logit to (max - 700) in fp32 first (one FMNMX; a double fmax costs five instructions):
+// terms that small cannot move a sum that is >= 1, and -inf logits never reach the fp64 code.
+// The full-width fp64 constants live in constant memory and are used as constant-bank operands: written as
+// literals, ptxas rebuilt each of them with two MOVs per use (47 instructions per element, issue-bound).
+__constant__ double kExpC[6] = {92.332482616893656,       // 64 / ln2
+                                -0.01083042469326756,      // -(ln2/64), high part: 32 significant bits
+                                -2.9815858269852933e-12,   // -(ln2/64), low part
+                                1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0};
+
 __device__ __forceinline__ double exp_neg(double d, const double* __restrict__ tab) {
-    if (d < -700.0) return 0.0;
     const double kMagic = 6755399441055744.0;                 // 2^52 + 2^51: round-to-nearest-integer by addition
-    const double t = fma(d, 92.332482616893656, kMagic);      // d * 64/ln2
+    const double t = fma(d, kExpC[0], kMagic);
     const int k = __double2loint(t);                          // integer in the low word (two's complement)
     const double kf = t - kMagic;
-    // r = d - k ln2/64 in two steps: the high part has 32 significant bits, so kf * hi is exact for |k| < 2^20
-    double r = fma(kf, -0.01083042469326756, d);
-    r = fma(kf, -2.9815858269852933e-12, r);
-    double p = fma(r, 1.0 / 120.0, 1.0 / 24.0);
-    p = fma(p, r, 1.0 / 6.0);
+    // r = d - k ln2/64 in two steps: kf * high part is exact for |k| < 2^20
+    double r = fma(kf, kExpC[1], d);
+    r = fma(kf, kExpC[2], r);
+    double p = fma(r, kExpC[3], kExpC[4]);
+    p = fma(p, r, kExpC[5]);
     p = fma(p, r, 0.5);
     p = fma(p, r, 1.0);
     p = fma(p, r, 1.0);
@@ -98,51 +105,8 @@ row_offset_kernel(const float* __restrict__ logits, const float* __restrict__ sc
     const int t = threadIdx.x % kTPR, r_in = threadIdx.x / kTPR;
     const float ninf = __int_as_float(0xff800000);
 
-    for (long long row0 = (long long)blockIdx.x * kRows; row0 < rows; row0 += (long long)gridDim.x * kRows) {
-        const long long row = row0 + r_in;
-        const bool live = row < rows;  // uniform per warp (kTPR >= 32)
-        const float* __restrict__ p = logits + (live ? row : 0) * (long long)C;
-        float m = ninf;
-        double s = 0.0;
-        if (vec) {
-            const float4* __restrict__ p4 = reinterpret_cast<const float4*>(p);
-            const int C4 = C >> 2;
-            float4 v[kRegVec];
-#pragma unroll
-            for (int x = 0; x < kRegVec; ++x) {
-                const int j = x * kTPR + t;
-                v[x] = make_float4(ninf, ninf, ninf, ninf);
-                if (live && j < C4) v[x] = __ldg(p4 + j);
-            }
-#pragma unroll
-            for (int x = 0; x < kRegVec; ++x) m = fmaxf(m, max4(v[x]));
-            if (live)
-                for (int j = kRegVec * kTPR + t; j < C4; j += kTPR) m = fmaxf(m, max4(__ldg(p4 + j)));
-            m = row_max<kTPR>(m, sm);
-            if (m != ninf) {  // uniform per row
-                const double md = (double)m;
-#pragma unroll
-                for (int x = 0; x < kRegVec; ++x) {
-                    if (x * kTPR + t < C4) {
-                        s += exp_neg((double)v[x].x - md, tab); s += exp_neg((double)v[x].y - md, tab);
-                        s += exp_neg((double)v[x].z - md, tab); s += exp_neg((double)v[x].w - md, tab);
-                    }
-                }
-                for (int j = kRegVec * kTPR + t; j < C4; j += kTPR) {
-                    const float4 w = __ldg(p4 + j);
-                    s += exp_neg((double)w.x - md, tab); s += exp_neg((double)w.y - md, tab);
-                    s += exp_neg((double)w.z - md, tab); s += exp_neg((double)w.w - md, tab);
-                }
-            }
-        } else {
-            if (live)
-                for (int j = t; j < C; j += kTPR) m = fmaxf(m, __ldg(p + j));
-            m = row_max<kTPR>(m, sm);
-            if (m != ninf) {
-                const double md = (double)m;
-                for (int j = t; j < C; j += kTPR) s += exp_neg((double)__ldg(p + j) - md, tab);
-            }
-        }
+    const long long stride = (long long)gridDim.x * kRows;
+    auto finish = [&](long long row, bool live, float m, double s) {
         s = row_sum<kTPR>(s, sd);
         if (live && t == 0) {
             float o = ninf;  // a beam without a legal continuation
@@ -152,6 +116,78 @@ row_offset_kernel(const float* __restrict__ logits, const float* __restrict__ sc
             }
             offset[row] = o;
         }
+    };
+
+    if (vec) {
+        // One row at a time per CTA, 64 registers, 4 CTAs per SM.  Measured at C = 8192 (B200, 134 MB): a register
+        // double buffer that requests the next row before this row's arithmetic needs 128 registers (2 CTAs per
+        // SM) and is slower (52.7 us against 49.6 us): the kernel is bound by fp64 issue, not by load latency.
+        const int C4 = C >> 2;
+        float4 nx[kRegVec];
+        auto load_row = [&](long long r0) {
+            const long long row = r0 + r_in;
+            const float4* __restrict__ p4 = reinterpret_cast<const float4*>(logits + (row < rows ? row : 0) * (long long)C);
+#pragma unroll
+            for (int x = 0; x < kRegVec; ++x) {
+                const int j = x * kTPR + t;
+                nx[x] = make_float4(ninf, ninf, ninf, ninf);
+                if (row < rows && j < C4) nx[x] = __ldg(p4 + j);
+            }
+        };
+        long long row0 = (long long)blockIdx.x * kRows;
+        for (; row0 < rows; row0 += stride) {
+            load_row(row0);
+            const long long row = row0 + r_in;
+            const bool live = row < rows;  // uniform per warp (kTPR >= 32)
+            const float4* __restrict__ p4 = reinterpret_cast<const float4*>(logits + (live ? row : 0) * (long long)C);
+            float4 v[kRegVec];
+#pragma unroll
+            for (int x = 0; x < kRegVec; ++x) v[x] = nx[x];
+            float m = ninf;
+#pragma unroll
+            for (int x = 0; x < kRegVec; ++x) m = fmaxf(m, max4(v[x]));
+            if (live)
+                for (int j = kRegVec * kTPR + t; j < C4; j += kTPR) m = fmaxf(m, max4(__ldg(p4 + j)));
+            m = row_max<kTPR>(m, sm);
+            double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+            if (m != ninf) {  // uniform per row
+                const double md = (double)m;
+                const float mlo = m - 700.f;
+#pragma unroll
+                for (int x = 0; x < kRegVec; ++x) {
+                    if (x * kTPR + t < C4) {
+                        s0 += exp_neg((double)fmaxf(v[x].x, mlo) - md, tab); s1 += exp_neg((double)fmaxf(v[x].y, mlo) - md, tab);
+                        s2 += exp_neg((double)fmaxf(v[x].z, mlo) - md, tab); s3 += exp_neg((double)fmaxf(v[x].w, mlo) - md, tab);
+                    }
+                }
+                for (int j = kRegVec * kTPR + t; j < C4; j += kTPR) {
+                    const float4 w = __ldg(p4 + j);
+                    s0 += exp_neg((double)fmaxf(w.x, mlo) - md, tab); s1 += exp_neg((double)fmaxf(w.y, mlo) - md, tab);
+                    s2 += exp_neg((double)fmaxf(w.z, mlo) - md, tab); s3 += exp_neg((double)fmaxf(w.w, mlo) - md, tab);
+                }
+            }
+            finish(row, live, m, (s0 + s1) + (s2 + s3));
+        }
+        return;
+    }
+
+    for (long long row0 = (long long)blockIdx.x * kRows; row0 < rows; row0 += stride) {
+        const long long row = row0 + r_in;
+        const bool live = row < rows;
+        const float* __restrict__ p = logits + (live ? row : 0) * (long long)C;
+        float m = ninf;
+        double s = 0.0;
+        {
+            if (live)
+                for (int j = t; j < C; j += kTPR) m = fmaxf(m, __ldg(p + j));
+            m = row_max<kTPR>(m, sm);
+            if (m != ninf) {
+                const double md = (double)m;
+                const float mlo = m - 700.f;
+                for (int j = t; j < C; j += kTPR) s += exp_neg((double)fmaxf(__ldg(p + j), mlo) - md, tab);
+            }
+        }
+        finish(row, live, m, s);
     }
 }
 
