@@ -62,6 +62,15 @@ def test_validation_before_cuda(L):
     assert L.stark_tree_attn_step(ctypes.byref(sh), p, 9, 1, p, p, p, p, p, p, 1, p, None) == -1   # n_q > Wmax
     assert L.stark_beam_topk(p, None, 1, 2, 4, 9, p, p, p, None, 0, None) == -1                    # W_out > W_in*C
     assert L.stark_beam_topk(p, None, 1, 1 << 16, 1 << 16, 4, p, p, p, None, 0, None) == -1        # >= 2^31
+    # selection from raw logits: same argument rules; the workspace (per-beam offsets) is mandatory
+    assert L.stark_beam_topk_logits(None, None, 1, 2, 4, 2, p, p, p, p, 1 << 20, None) == -1        # logits missing
+    assert L.stark_beam_topk_logits(p, None, 1, 2, 4, 9, p, p, p, p, 1 << 20, None) == -1          # W_out > W_in*C
+    assert L.stark_beam_topk_logits(p, None, 1, 2, 4, 2, p, p, p, None, 0, None) == -3             # no workspace
+    assert L.stark_beam_topk_logits(p, None, 1, 2, 4, 2, p, p, p, p, 8, None) == -3                # too small
+    assert L.stark_logits_row_offset(p, None, 0, 4, p, None) == -1                                 # rows < 1
+    assert L.stark_logits_row_offset(p, None, 4, 4, None, None) == -1                              # offset missing
+    need = L.stark_workspace_bytes(ctypes.byref(sh), sb.CALL_BEAM_TOPK_LOGITS, 8, 32)
+    assert need >= 1 * 8 * 4 and need % 256 == L.stark_workspace_bytes(ctypes.byref(sh), sb.CALL_BEAM_TOPK, 8, 32) % 256
     assert L.stark_kv_append_reorg(ctypes.byref(sh), 0, 1, p, p, p, p, p, p, None) == -1           # level < 1
     assert L.stark_kv_append_reorg(ctypes.byref(sh), 2, 1, p, p, None, p, p, p, None) == -1        # parent missing
     # fused decode attention: argument errors first, then "bf16 only" (fp32 shapes compose A1 + A2)
