@@ -265,7 +265,9 @@ int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_
  *
  * stark_logits_row_offset is the first half on its own (rows = B*W_in beams,
  * logits [rows, C] fp32, score [rows] fp32 or NULL => zeros, offset out [rows]).
- * stark_beam_topk_logits runs both; ws, ws_bytes = workspace of
+ * stark_beam_topk_logits runs both (one launch when W_in == 1 and C <= 512, i.e.
+ * decode step 0: the one-CTA selection kernel normalises its single row itself;
+ * two launches otherwise); ws, ws_bytes = workspace of
  * stark_workspace_bytes(shape (B only), STARK_CALL_BEAM_TOPK_LOGITS, W_in, C).
  * Errors: as stark_beam_topk; the workspace is always required.
  */

@@ -299,6 +299,9 @@ int stark_beam_topk_logits(const float* logits, const float* score_or_null, int 
     if (!ws || ws_bytes < off_bytes + tk_bytes) return STARK_ERR_WORKSPACE;
     int rc = check_device();
     if (rc != STARK_OK) return rc;
+    if (topk_can_fold_lse(W_in, C))  // decode step 0: the one-CTA kernel normalises its single row itself
+        return launch_topk(logits, score_or_null, B, W_in, C, W_out, out_score, out_parent, out_code,
+                           static_cast<char*>(ws) + off_bytes, ws_bytes - off_bytes, (cudaStream_t)stream, true);
     float* offset = static_cast<float*>(ws);
     rc = launch_row_offset(logits, score_or_null, (long long)B * W_in, C, offset, (cudaStream_t)stream);
     if (rc != STARK_OK) return rc;

@@ -107,7 +107,10 @@ int launch_append(const Dims& p, int dtype, int level, int n_new, const void* kn
                   const int32_t* parent, void* ks, void* vs, int32_t* anc, cudaStream_t st);
 int launch_topk(const float* logp, const float* score, int B, int W_in, int C, int W_out,
                 float* out_score, int32_t* out_parent, int32_t* out_code, void* ws, size_t ws_bytes,
-                cudaStream_t st);
+                cudaStream_t st, bool fold_lse = false);
+// fold_lse: `logp` holds RAW logits and the kernel folds the row's log-sum-exp into the score itself (reading
+// R22); only where topk_can_fold_lse() says so (one row per user, small enough for the one-CTA kernel).
+bool topk_can_fold_lse(int W_in, int C);
 size_t topk_workspace_bytes(int B, int W_in, int C);
 int launch_row_offset(const float* logits, const float* score, long long rows, int C, float* offset,
                       cudaStream_t st);

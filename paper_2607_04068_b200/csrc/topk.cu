@@ -702,7 +702,10 @@ topk_kernel(const float* __restrict__ logp, const float* __restrict__ score, int
 constexpr int kSmallMax = 512;       // beyond this the N^2 / 2 compares cost more than the radix passes
 constexpr int kSmallThreads = 256;
 
-template <int PER>  // candidates per thread
+// kFold (W_in == 1 only: decode step 0, the user's single row IS the candidate set): the input holds RAW logits
+// and the log-softmax normaliser is folded into the score here (reading R22, as logits_offset.cu does for
+// general shapes): offset = fl32(score - fl32(logsumexp(row))), fp64 sum -- no separate launch.
+template <int PER, bool kFold>  // candidates per thread
 __global__ void __launch_bounds__(kSmallThreads)
 topk_small_kernel(const float* __restrict__ logp, const float* __restrict__ score, int W_in, int C, int W_out,
                   float* __restrict__ out_score, int32_t* __restrict__ out_parent, int32_t* __restrict__ out_code) {
@@ -720,10 +723,40 @@ topk_small_kernel(const float* __restrict__ logp, const float* __restrict__ scor
         row[x] = idx / C;
         key[x] = __ldg(lp + idx);
     }
+    float fold_off = 0.f;
+    if constexpr (kFold) {
+        __shared__ float fm[kSmallThreads / 32];
+        __shared__ double fs[kSmallThreads / 32];
+        const float ninf = __int_as_float(0xff800000);
+        float m = ninf;
+#pragma unroll
+        for (int x = 0; x < PER; ++x) if (tid + x * kSmallThreads < N) m = fmaxf(m, key[x]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if ((tid & 31) == 0) fm[tid >> 5] = m;
+        __syncthreads();
+        m = fm[0];
+#pragma unroll
+        for (int w = 1; w < kSmallThreads / 32; ++w) m = fmaxf(m, fm[w]);
+        double s = 0.0;
+        if (m != ninf) {
+#pragma unroll
+            for (int x = 0; x < PER; ++x)
+                if (tid + x * kSmallThreads < N) s += exp((double)key[x] - (double)m);   // exp(-inf) = 0
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if ((tid & 31) == 0) fs[tid >> 5] = s;
+        __syncthreads();
+        s = fs[0];
+#pragma unroll
+        for (int w = 1; w < kSmallThreads / 32; ++w) s += fs[w];
+        fold_off = m == ninf ? ninf : __fsub_rn(sc ? __ldg(sc) : 0.f, __double2float_rn((double)m + log(s)));
+    }
 #pragma unroll
     for (int x = 0; x < PER; ++x) {
         const int idx = tid + x * kSmallThreads;
-        key[x] = __fadd_rn(sc ? __ldg(sc + row[x]) : 0.f, key[x]);
+        key[x] = __fadd_rn(kFold ? fold_off : (sc ? __ldg(sc + row[x]) : 0.f), key[x]);
         mine[x] = idx < N ? (((unsigned long long)(~ord_of(key[x])) << 32) | (uint32_t)idx) : ~0ull;
         comp[idx] = mine[x];
         rk[x] = 0;
@@ -960,15 +993,23 @@ int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
 
 size_t topk_workspace_bytes(int, int, int) { return 0; }
 
+bool topk_can_fold_lse(int W_in, int C) { return W_in == 1 && C <= kSmallMax; }
+
 int launch_topk(const float* logp, const float* score, int B, int W_in, int C, int W_out,
                 float* out_score, int32_t* out_parent, int32_t* out_code, void*, size_t,
-                cudaStream_t st) {
+                cudaStream_t st, bool fold_lse) {
     const long long N = (long long)W_in * C;
+    if (fold_lse && !topk_can_fold_lse(W_in, C)) return STARK_ERR_INVALID_ARG;
     if (N <= kSmallMax) {
-        if (N <= kSmallThreads)
-            topk_small_kernel<1><<<B, kSmallThreads, 0, st>>>(logp, score, W_in, C, W_out, out_score, out_parent, out_code);
+        if (fold_lse) {
+            if (N <= kSmallThreads)
+                topk_small_kernel<1, true><<<B, kSmallThreads, 0, st>>>(logp, score, W_in, C, W_out, out_score, out_parent, out_code);
+            else
+                topk_small_kernel<2, true><<<B, kSmallThreads, 0, st>>>(logp, score, W_in, C, W_out, out_score, out_parent, out_code);
+        } else if (N <= kSmallThreads)
+            topk_small_kernel<1, false><<<B, kSmallThreads, 0, st>>>(logp, score, W_in, C, W_out, out_score, out_parent, out_code);
         else
-            topk_small_kernel<2><<<B, kSmallThreads, 0, st>>>(logp, score, W_in, C, W_out, out_score, out_parent, out_code);
+            topk_small_kernel<2, false><<<B, kSmallThreads, 0, st>>>(logp, score, W_in, C, W_out, out_score, out_parent, out_code);
         STARK_LAUNCH_CHECK();
         return STARK_OK;
     }

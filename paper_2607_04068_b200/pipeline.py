@@ -49,7 +49,7 @@ class DecodePass:
     @property
     def launches(self) -> int:
         return ((2 if self.fused else 3) * self.d + (0 if self.inline_append else self.d - 1)
-                + (self.d if self.from_logits else 0))
+                + (sum(1 for t in range(self.d) if not (self.n_q[t] == 1 and self.C <= 512)) if self.from_logits else 0))
 
     def run(self) -> None:
         score = parent = None

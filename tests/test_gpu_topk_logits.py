@@ -46,6 +46,19 @@ def test_random_logits(B, W_in, C, W_out):
     _check(logits, score, W_out)
 
 
+@pytest.mark.parametrize("B,C,W_out", [(2, 400, 100), (1, 512, 512), (3, 257, 64), (16, 256, 64), (2, 7, 7)])
+def test_single_row_folded_in_the_one_cta_kernel(B, C, W_out):
+    """W_in = 1, C <= 512 (decode step 0): the one-CTA top-k kernel folds the log-sum-exp itself (no row-offset
+    launch); one and two candidates per thread, with and without a root score, -inf masks, a dead user."""
+    r = _rng(6)
+    logits = r.normal(0, 2, (B, 1, C)).astype(np.float32)
+    _check(logits, None, W_out)
+    _check(logits, r.normal(-2, 1, (B, 1)).astype(np.float32), W_out)
+    logits[:, :, C // 2:] = -np.inf
+    logits[0] = -np.inf
+    _check(logits, r.normal(-2, 1, (B, 1)).astype(np.float32), W_out)
+
+
 def test_mixture_near_ties_and_large_offsets():
     """Config 4's mixture (90 % N(0,1), 10 % N(3, 0.5)) plus a large common shift per beam: the max subtraction
     must keep the fp64 sum exact enough for a correctly rounded fp32 lse."""
