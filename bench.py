@@ -557,7 +557,7 @@ def run_stark(args, cfg):
     e2e_ms = (time.perf_counter() - t0) * 1e3 / n_e2e
     e2e = {"value": world * sids_per_pass / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": n_e2e,
-           "note": "prefix K/V + per-step q/k/v/log-probs copied from pinned host memory every pass; "
+           "note": "prefix K/V + per-step q/k/v/log-probs (raw logits with --from-logits) copied from pinned host memory every pass; "
                    "per-level (score,parent,code) read back; two input sets in turn, the copy of pass i+1 "
                    "overlaps pass i (wall clock, host waits for every result)"}
 
