@@ -30,7 +30,7 @@ def test_full_size_parity(name):
     assert not bad, f"{name}: {bad}\nfull report: {rep}"
 
 
-@pytest.mark.parametrize("name", ["cfg2", "cfg4"])
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5", "paper_b1"])
 def test_full_size_parity_from_logits(name):
     """The same pass with the selection fed RAW logits (stark_beam_topk_logits, reading R22; bench.py
     --from-logits): every level's (score, parent, code) bit-exact vs oracle.select_beams_from_logits, the
