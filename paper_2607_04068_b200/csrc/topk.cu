@@ -11,6 +11,8 @@
 // W_out <= 256: one 1024-thread CTA per user, bound from per-thread maxima +
 // ranking by counting (topk_mid_kernel); otherwise the cluster kernel described
 // here (topk_kernel).  All three produce the same total order.
+// stark_beam_topk_logits (reading R22) feeds the same kernels (raw logits, per-beam offset from
+// logits_offset.cu); for a single-row user the small kernel computes that offset itself (kFold).
 //
 // The work is tiny next to its latency (1 MB per level at config 2), so the
 // design minimises dependent phases and cross-CTA traffic (measured on B200: a
