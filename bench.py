@@ -241,7 +241,9 @@ def whole_job_value(world: int, sids_per_pass: int, ms_per_step: float) -> float
 def run_calibrate():
     """Launch floor and plain cold-stream floors (one graph of 24 launches rotating over buffers > L2)."""
     import torch
-    from paper_2607_04068_b200 import binding as sb
+    from paper_2607_04068_b200.build import build
+    from paper_2607_04068_b200 import calib as sb
+    build()
     sb.lib()
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(0)
@@ -257,12 +259,11 @@ def run_calibrate():
 
 
 def run_cfg3_decoder(args):
-    """BASELINE configs[2]: the library inside a 12-layer random-init decoder (tests/_decoder_harness.py; GEMMs in
+    """BASELINE configs[2]: the library inside a 12-layer random-init decoder (paper_2607_04068_b200/decoder_harness.py; GEMMs in
     torch/cuBLAS, not graded).  Prefill untimed.  Reports the whole decode (4 levels x 12 layers) and the
     library calls alone (same captured inputs, no GEMMs), eager launches, CUDA events."""
     import torch
-    sys.path.insert(0, os.path.join(ROOT, "tests"))
-    from _decoder_harness import Decoder, DecoderShape
+    from paper_2607_04068_b200.decoder_harness import Decoder, DecoderShape
     sh = DecoderShape()
     model = Decoder(sh, seed=0)
     g = torch.Generator(device="cpu").manual_seed(3)

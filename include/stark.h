@@ -138,9 +138,12 @@ int stark_prefix_attn(const stark_shape_t* shape, const void* q, int n_q,
                       int n_splits, float* part_m, float* part_l, float* part_o,
                       void* ws, size_t ws_bytes, void* stream);
 
-/* Deterministic, shape-only choice of n_splits (host arithmetic, no CUDA
- * call): 1 when the (user, KV head, M tile) grid alone fills the GPU, more
- * when it does not (step 0, small batches).  Writes *n_splits (host). */
+/* Deterministic choice of n_splits from the shapes and the SM count of the
+ * CURRENT device (one cudaGetDevice / cudaDeviceGetAttribute query, cached per
+ * device; 148 is assumed when no device is present; no launch, no
+ * synchronisation): 1 when the (user, KV head, M tile) grid alone fills the
+ * GPU, more when it does not (step 0, small batches).  Writes *n_splits (host).
+ * Call it with the device current on which stark_prefix_attn will run. */
 int stark_prefix_attn_plan(const stark_shape_t* shape, int n_q, int total_tokens,
                            int max_prefix_len, int* n_splits);
 
@@ -313,18 +316,6 @@ size_t stark_workspace_bytes(const stark_shape_t* shape, int call, int n_q, int 
 size_t stark_suffix_bytes(const stark_shape_t* shape);
 /* Bytes of anc: 2*B*Wmax*d*4. */
 size_t stark_anc_bytes(const stark_shape_t* shape);
-
-/* ---------------------------------------------------------------------------
- * Measurement aids (used by `bench.py --calibrate`; not part of the method).
- * stark_calib_empty: launches an empty kernel -- the launch floor.
- * stark_calib_stream_read: a plain grid-stride 16-byte read of `bytes` bytes of
- * device memory `src` (148*8 CTAs of 256 threads, 4 loads in flight per thread)
- * -- what a trivial HBM-bound kernel of that size achieves, launch and ramp
- * included; sink must point to 4 writable device bytes (never written unless
- * the data XORs to a magic value).  Errors: INVALID_ARG, CUDA.
- */
-int stark_calib_empty(void* stream);
-int stark_calib_stream_read(const void* src, size_t bytes, void* sink, void* stream);
 
 int stark_version(void);
 /* Static string describing a stark_status_t. */

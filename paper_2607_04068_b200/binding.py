@@ -23,7 +23,6 @@ EXPORTS = (
     "stark_beam_topk", "stark_logits_row_offset", "stark_beam_topk_logits",
     "stark_kv_append_reorg", "stark_workspace_bytes", "stark_suffix_bytes",
     "stark_anc_bytes", "stark_version", "stark_status_string", "stark_last_cuda_error",
-    "stark_calib_empty", "stark_calib_stream_read",
 )
 
 
@@ -85,10 +84,6 @@ def lib() -> ctypes.CDLL:
     L.stark_suffix_bytes.argtypes = [P]
     L.stark_anc_bytes.restype = c_size_t
     L.stark_anc_bytes.argtypes = [P]
-    L.stark_calib_empty.restype = c_int
-    L.stark_calib_empty.argtypes = [c_void_p]
-    L.stark_calib_stream_read.restype = c_int
-    L.stark_calib_stream_read.argtypes = [c_void_p, c_size_t, c_void_p, c_void_p]
     L.stark_version.restype = c_int
     L.stark_status_string.restype = ctypes.c_char_p
     L.stark_status_string.argtypes = [c_int]
@@ -205,14 +200,6 @@ def stark_kv_append_reorg(shape: Shape, level: int, n_new: int, k_new: torch.Ten
     _check(lib().stark_kv_append_reorg(byref(shape), level, n_new, _ptr(k_new), _ptr(v_new), _ptr(parent),
                                        _ptr(k_suffix), _ptr(v_suffix), _ptr(anc), _stream()),
            "stark_kv_append_reorg")
-
-
-def stark_calib_empty() -> None:
-    _check(lib().stark_calib_empty(_stream()), "stark_calib_empty")
-
-
-def stark_calib_stream_read(src: torch.Tensor, nbytes: int, sink: torch.Tensor) -> None:
-    _check(lib().stark_calib_stream_read(_ptr(src), nbytes, _ptr(sink), _stream()), "stark_calib_stream_read")
 
 
 def stark_workspace_bytes(shape: Shape, call: int, n_q: int, total_tokens: int) -> int:

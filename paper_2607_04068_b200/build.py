@@ -18,6 +18,9 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB_PATH = os.path.join(HERE, "libstark.so")
 OBJ_DIR = os.path.join(HERE, "build")
+# bench-only measurement aids (calib/stark_calib.h): a library of their own, outside the product ABI
+CALIB_DIR = os.path.join(HERE, "calib")
+CALIB_LIB = os.path.join(CALIB_DIR, "libstark_calib.so")
 
 SOURCES = ["api.cu", "append.cu", "tree_attn.cu", "prefix_simt.cu", "prefix_tc.cu", "topk.cu", "logits_offset.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
@@ -32,10 +35,11 @@ def _nvcc() -> str:
 
 
 def _stale() -> bool:
-    if not os.path.exists(LIB_PATH):
+    if not os.path.exists(LIB_PATH) or not os.path.exists(CALIB_LIB):
         return True
-    t = os.path.getmtime(LIB_PATH)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(INCLUDE, "stark.h"), __file__]
+    t = min(os.path.getmtime(LIB_PATH), os.path.getmtime(CALIB_LIB))
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(INCLUDE, "stark.h"), __file__] \
+        + [os.path.join(CALIB_DIR, f) for f in ("calib.cu", "stark_calib.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
@@ -63,6 +67,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)
         raise RuntimeError("nvcc link failed")
+    cmd = [nvcc, *ARCH, "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", CALIB_DIR, "-shared",
+           "-o", CALIB_LIB, os.path.join(CALIB_DIR, "calib.cu")]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError("nvcc failed on calib.cu")
     return LIB_PATH
 
 

@@ -11,36 +11,44 @@ int& last_cuda_error_ref() {
     return e;
 }
 
+int current_device() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return 0; }
+    return dev < 0 ? 0 : (dev >= kMaxDevices ? kMaxDevices - 1 : dev);
+}
+
 int num_sms() {
-    static int n = 0;
-    if (n == 0) {
+    static PerDevice<int> n;
+    int& c = n.here();
+    if (c == 0) {
         int dev = 0, v = 0;
         if (cudaGetDevice(&dev) == cudaSuccess &&
             cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
-            n = v;
+            c = v;
         else {
             (void)cudaGetLastError();
             return 148;  // B200; used for planning only
         }
     }
-    return n;
+    return c;
 }
 
 namespace {
 
-// 0 = unknown, 1 = sm_100, -1 = something else / no device
+// per device: 0 = unknown, 1 = sm_100, -1 = something else; -2 (not cached) = no device
 int device_ok() {
-    static int state = 0;
-    if (state == 0) {
+    static PerDevice<int> state;
+    int& s = state.here();
+    if (s == 0) {
         int dev = 0, major = 0;
         if (cudaGetDevice(&dev) != cudaSuccess ||
             cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
             last_cuda_error_ref() = (int)cudaGetLastError();
             return -2;
         }
-        state = major == 10 ? 1 : -1;
+        s = major == 10 ? 1 : -1;
     }
-    return state;
+    return s;
 }
 
 int check_shape(const stark_shape_t* s) {
@@ -250,19 +258,6 @@ int stark_decode_step(const stark_shape_t* shape, const void* q, int n_q, int le
                                plan_cluster_splits(p, n_q, max_prefix_len), k_suffix, v_suffix, anc_prev, out,
                                (cudaStream_t)stream, level >= 1 ? k_new : nullptr, level >= 1 ? v_new : nullptr, parent,
                                anc_new);
-}
-
-int stark_calib_empty(void* stream) {
-    const int rc = check_device();
-    if (rc != STARK_OK) return rc;
-    return launch_calib(nullptr, 0, nullptr, (cudaStream_t)stream);
-}
-
-int stark_calib_stream_read(const void* src, size_t bytes, void* sink, void* stream) {
-    if (!src || !sink || bytes < 16) return STARK_ERR_INVALID_ARG;
-    const int rc = check_device();
-    if (rc != STARK_OK) return rc;
-    return launch_calib(src, bytes, sink, (cudaStream_t)stream);
 }
 
 int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_in, int C, int W_out,

@@ -63,33 +63,7 @@ append_kernel(const uint4* __restrict__ kn, const uint4* __restrict__ vn, uint4*
     }
 }
 
-// ---- measurement aids (stark_calib_*): launch floor and plain cold-stream floor -----------------
-__global__ void calib_empty_kernel() {}
-
-__global__ void __launch_bounds__(kThreads)
-calib_read_kernel(const uint4* __restrict__ p, size_t n, int* sink) {
-    uint4 acc = make_uint4(0, 0, 0, 0);
-    size_t i = (size_t)blockIdx.x * kThreads + threadIdx.x;
-    const size_t stride = (size_t)gridDim.x * kThreads;
-#pragma unroll 4
-    for (; i < n; i += stride) {
-        const uint4 v = __ldg(p + i);
-        acc.x ^= v.x; acc.y ^= v.y; acc.z ^= v.z; acc.w ^= v.w;
-    }
-    if ((acc.x ^ acc.y ^ acc.z ^ acc.w) == 0x5a17c0deu) *sink = 1;  // keeps the loads alive
-}
-
 }  // namespace
-
-int launch_calib(const void* src, size_t bytes, void* sink, cudaStream_t st) {
-    if (!src) {
-        calib_empty_kernel<<<1, 32, 0, st>>>();
-    } else {
-        calib_read_kernel<<<148 * 8, kThreads, 0, st>>>((const uint4*)src, bytes / 16, (int*)sink);
-    }
-    STARK_LAUNCH_CHECK();
-    return STARK_OK;
-}
 
 int launch_append(const Dims& p, int dtype, int level, int n_new, const void* kn, const void* vn,
                   const int32_t* parent, void* ks, void* vs, int32_t* anc, cudaStream_t st) {

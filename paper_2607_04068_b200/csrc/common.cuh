@@ -41,7 +41,16 @@ int& last_cuda_error_ref();
 
 #define STARK_LAUNCH_CHECK() STARK_CUDA_TRY(cudaGetLastError())
 
-int num_sms();  // cached cudaDevAttrMultiProcessorCount (148 on B200); <=0 on failure
+// cudaFuncSetAttribute, occupancy and SM count are PER DEVICE: every cached value is keyed by the current
+// device (cudaGetDevice), so that a process driving several GPUs gets each of them set up.
+constexpr int kMaxDevices = 64;
+int current_device();  // cudaGetDevice(), clamped to [0, kMaxDevices); 0 if the call fails
+template <typename T>
+struct PerDevice {
+    T v[kMaxDevices] = {};
+    T& here() { return v[current_device()]; }
+};
+int num_sms();  // cudaDevAttrMultiProcessorCount of the current device, cached per device (148 on B200)
 
 // ---- element access ---------------------------------------------------------
 template <typename T> struct Elem;
@@ -114,6 +123,5 @@ bool topk_can_fold_lse(int W_in, int C);
 size_t topk_workspace_bytes(int B, int W_in, int C);
 int launch_row_offset(const float* logits, const float* score, long long rows, int C, float* offset,
                       cudaStream_t st);
-int launch_calib(const void* src_or_null, size_t bytes, void* sink, cudaStream_t st);
 
 }  // namespace stark

@@ -950,11 +950,11 @@ bool make_map(CUtensorMap* tm, const void* base, int D, int n1, long long n2, in
 template <int D>
 int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, int n_q,
              const int32_t* cu, int n_splits, float* pm, float* pl, float* po, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
+    static PerDevice<bool> attr_done;
+    if (!attr_done.here()) {
         STARK_CUDA_TRY(cudaFuncSetAttribute(prefix_tc_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             TcCfg<D>::SMEM_BYTES));
-        attr_done = true;
+        attr_done.here() = true;
     }
     const int M = n_q * p.G;
     const int parity = prefix_tc_parity(p, n_q, n_splits) ? 1 : 0;
@@ -970,11 +970,11 @@ int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const 
 template <int D>
 int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, int n_q,
                    const int32_t* cu, int n_splits, const FusedArgs& fa, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
+    static PerDevice<bool> attr_done;
+    if (!attr_done.here()) {
         STARK_CUDA_TRY(cudaFuncSetAttribute(prefix_tc_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             TcCfg<D>::SMEM_BYTES));
-        attr_done = true;
+        attr_done.here() = true;
     }
     const int M = n_q * p.G;
     const int parity = prefix_tc_parity(p, n_q, n_splits) ? 1 : 0;

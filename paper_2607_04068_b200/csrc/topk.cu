@@ -81,6 +81,7 @@ constexpr int kSliceMin = 2048;       // do not split a user into slices smaller
 constexpr int kRankSortMax = 256;    // up to here a counting rank sort beats the bitonic network
 constexpr int kRegSortMax = 1024;     // sorted runs of 64 per warp + merge by ranking
 constexpr int kSmemBudget = 227 * 1024;
+constexpr int kMinCacheKeys = 8192;   // smallest key cache worth launching with (launch_topk)
 
 struct Shared {
     uint32_t hist[2][kBins];       // ping-pong by pass parity
@@ -1018,7 +1019,8 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
     // (measured: W_out = 512 of 8192 candidates, 20 us against 15 us for the cluster kernel; 32 K candidates with
     // 32 per thread, 13.1 against 12.8 us: two cold load rounds)
     if (N <= kMidMaxN && W_out <= kMidUseK) {
-        static bool mid_attr_done = false;
+        static PerDevice<bool> mid_attr;
+        bool& mid_attr_done = mid_attr.here();
         if (!mid_attr_done) {
             STARK_CUDA_TRY(cudaFuncSetAttribute(topk_mid_kernel<kMidKeysPerThread>,
                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, kMidMaxN * 4));
@@ -1033,10 +1035,18 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
     }
     const int cap = next_pow2(W_out) * 2 < 128 ? 128 : next_pow2(W_out) * 2;  // sort buffer entries
     // pruning pays once a thread holds many keys (>= 16: slices of 8192) and needs K <= the 2048 buckets of a CTA
-    const int prune = (N / kMaxCluster >= 8192 || N >= 32768) && W_out <= 2048 ? 1 : 0;
-    const size_t fixed = ((sizeof(Shared) + 15) / 16) * 16 + (size_t)cap * 8 * (prune ? 9 : 1);  // sel + 2 lists of 4 * cap
+    int prune = (N / kMaxCluster >= 8192 || N >= 32768) && W_out <= 2048 ? 1 : 0;
+    auto fixed_bytes = [&](int pr) {  // Shared + sel (+ the two survivor lists of 4 * cap entries when pruning)
+        return ((sizeof(Shared) + 15) / 16) * 16 + (size_t)cap * 8 * (pr ? 9 : 1);
+    };
+    // the survivor lists of a wide selection (1024 < W_out <= 2048: cap = 4096, 288 KB) do not fit next to a
+    // useful key cache: select without pruning then (the slice beyond the cache is re-read through L2)
+    if (prune && (long long)kSmemBudget - (long long)fixed_bytes(1) < (long long)kMinCacheKeys * 4) prune = 0;
+    const size_t fixed = fixed_bytes(prune);
     const long long cache_max = ((long long)kSmemBudget - (long long)fixed) / 4;
-    static bool attr_done = false;  // idempotent; a benign race at worst repeats the calls
+    if (cache_max < kMinCacheKeys) return STARK_ERR_UNSUPPORTED;  // (unreachable for W_out <= 4096)
+    static PerDevice<bool> attr;  // idempotent; a benign race at worst repeats the calls
+    bool& attr_done = attr.here();
     if (!attr_done) {
         STARK_CUDA_TRY(cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBudget));
         STARK_CUDA_TRY(cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
@@ -1061,7 +1071,10 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
         at[0].val.clusterDim.x = n;
     };
     auto max_clusters = [&](int n) -> int {  // resident clusters of size n with the current smem; cached
-        static int memo_smem[5] = {-1, -1, -1, -1, -1}, memo_val[5] = {0, 0, 0, 0, 0};
+        struct Memo { int smem[5], val[5]; };
+        static PerDevice<Memo> memo;  // (zero-initialised: no launch has 0 bytes of dynamic shared memory)
+        int* memo_smem = memo.here().smem;
+        int* memo_val = memo.here().val;
         int slot = 0;
         while ((1 << slot) < n) ++slot;
         if (memo_smem[slot] != (int)cfg.dynamicSmemBytes) {

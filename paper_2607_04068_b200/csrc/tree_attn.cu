@@ -227,7 +227,8 @@ int launch_m(const Dims& p, const void* q, int n_q, int level, const void* ks, c
     const unsigned nb = (unsigned)((warps + kWarpsPerCta - 1) / kWarpsPerCta);
     const size_t smem = kWarpsPerCta * warp_region_bytes(hpw, D, (int)sizeof(T), level);
     if (smem > 48 * 1024) {
-        static size_t opted = 0;  // idempotent; a benign race at worst repeats the call
+        static PerDevice<size_t> opted_dev;  // idempotent; a benign race at worst repeats the call
+        size_t& opted = opted_dev.here();
         if (smem > 227 * 1024) return STARK_ERR_UNSUPPORTED;
         if (smem > opted) {
             STARK_CUDA_TRY(cudaFuncSetAttribute(tree_attn_kernel<T, D, ML>, cudaFuncAttributeMaxDynamicSharedMemorySize,

@@ -1,6 +1,7 @@
 """Config 3 harness (BASELINE.json configs[2]; reading R17): a random-init decoder-only transformer
 whose GEMMs run in torch/cuBLAS while decode attention, KV append/reorg and beam top-k go through the STARK
-library.  TEST INFRASTRUCTURE: it shows the four calls inside a real multi-layer decode loop (the tree is
+library.  A USER of the library, not part of its hot path (it lives in the package so that both `bench.py
+--workload cfg3_decoder` and `tests/` can import it): it shows the four calls inside a real multi-layer decode loop (the tree is
 shared by all layers: layer 0 writes the ancestor index, the others pass write_anc = 0) and captures per-call
 inputs so that tests can compare sampled (layer, user, step) triples with the oracle.
 
@@ -16,7 +17,7 @@ from typing import Dict, List
 import torch
 import torch.nn.functional as F
 
-from paper_2607_04068_b200.decode import StarkLayer, beam_topk
+from .decode import StarkLayer, beam_topk
 
 
 @dataclass

@@ -125,11 +125,11 @@ def run_full_size(cfg, n_samples=6, seed=0, use_graph=True, from_logits=False):
     """Free-running DecodePass (bench.py's own object, CUDA-graph replay) at BASELINE.json's full size.
     Checks: (a) every level's selection, ALL users, bit-exact vs oracle.select_beams on the identical fp32
     log-probs and scores; (b) the ancestor index vs oracle.ancestor_chains and the suffix K/V (bitwise copy);
-    (c) attention rows of sampled (user, beam) pairs vs oracle.replay_beam_attention (conventional
-    per-beam full-sequence attention, fp64); (d) the prefix buffers are bit-identical before/after."""
+    (c) ALL attention rows of whole users (first, last, shortest, longest prefix) vs
+    oracle.sequence_expanded_attention (fp64) plus sampled rows of other users vs the per-beam replay; (d) the prefix buffers are bit-identical before/after."""
     import bench
     from oracle.selection import select_beams, select_beams_from_logits
-    from oracle.tree import ancestor_chains
+    from oracle.tree import ancestor_chains, sequence_expanded_attention
     from oracle.replay import replay_beam_attention
     h = bench.host_inputs(cfg, seed)
     p = bench.make_pass(cfg, h, torch.device("cuda"), from_logits=from_logits)
@@ -177,10 +177,22 @@ def run_full_size(cfg, n_samples=6, seed=0, use_graph=True, from_logits=False):
             report.append(("append_kv_bitwise", t, bool(ok_kv), ""))
             if t + 2 > cfg.d - 1:      # anc ping-pongs by level parity: level t's half is reused by level t+2
                 report.append(("anc_vs_oracle_chains", t, bool(ok_anc), ""))
-        # (c) sampled attention rows.  NOTE: after the whole pass anc/suffix hold the final state; level-t
-        # rows are never overwritten by later levels, so every step can be checked afterwards.
+        # (c) attention, ALL rows of whole users (first, last, shortest and longest prefix) vs the oracle's
+        # sequence-expanded masked attention (Eq. 14, oracle/tree.py; pinned equal to the conventional per-beam
+        # form), plus a few sampled (user, beam) rows of the other users vs the conventional per-beam replay.
+        # NOTE: after the whole pass anc/suffix hold the final state; level-t rows are never overwritten by
+        # later levels, so every step can be checked afterwards.
         out = p.out[t].float().cpu().numpy().astype(np.float64)
         worst, ref_max = 0.0, 0.0
+        lens = np.diff(cu)
+        whole = sorted({0, cfg.B - 1, int(np.argmin(lens)), int(np.argmax(lens))})
+        for u in whole:
+            parents = [sel[l][1][u] for l in range(t)]
+            ref = sequence_expanded_attention(h["K"][cu[u]:cu[u + 1]], h["V"][cu[u]:cu[u + 1]],
+                                              [h["k"][l][u] for l in range(1, t + 1)],
+                                              [h["v"][l][u] for l in range(1, t + 1)], parents, h["q"][t][u], t, scale)
+            worst = max(worst, float(np.abs(out[u] - ref).max()))
+            ref_max = max(ref_max, float(np.abs(ref).max()))
         for _ in range(n_samples):
             u, i = int(rng.integers(cfg.B)), int(rng.integers(p.n_q[t]))
             parents = [sel[l][1][u] for l in range(t)]
@@ -189,6 +201,6 @@ def run_full_size(cfg, n_samples=6, seed=0, use_graph=True, from_logits=False):
                                         parents, h["q"][t][u, i], i, t, scale)
             worst = max(worst, float(np.abs(out[u, i] - ref).max()))
             ref_max = max(ref_max, float(np.abs(ref).max()))
-        report.append(("attn_sampled", t, bool(np.isfinite(out).all() and worst <= tol * ref_max),
-                       f"max_abs_err={worst:.3e} max|ref|={ref_max:.3e} tol={tol}"))
+        report.append(("attn_whole_users", t, bool(np.isfinite(out).all() and worst <= tol * ref_max),
+                       f"users={whole} (+{n_samples} sampled rows) max_abs_err={worst:.3e} max|ref|={ref_max:.3e} tol={tol}"))
     return report

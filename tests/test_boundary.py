@@ -88,7 +88,6 @@ def test_validation_before_cuda(L):
     assert step(bf, p, 1, 1, p, p, p, 4, 4, None, p, None, p, p, p, 1, p, None) == -1                # k_new missing
     assert step(bf, p, 1, 2, p, p, p, 4, 4, p, p, None, p, p, p, 0, p, None) == -1                   # parent missing
     assert step(sh, p, 1, 0, p, p, p, 4, 4, None, None, None, None, None, None, 1, p, None) == -2    # fp32
-    assert L.stark_calib_stream_read(None, 64, p, None) == -1
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="only meaningful without a GPU")

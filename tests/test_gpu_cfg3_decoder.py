@@ -4,6 +4,7 @@ Per-call parity on captured inputs ("Config 3: sampled (
     position in every layer (an independent library routine as reference);
   * sampled (layer, user, step, beam): attention row vs the oracle's conventional per-beam full-sequence
     attention over that layer's captured prefix + suffix K/V and the selected parents;
+  * ALL beams of two whole (layer, user) pairs at every step vs the oracle's sequence-expanded Eq.-14 attention;
   * every level's selection bit-exact vs oracle.select_beams on the captured fp32 log-probs and scores."""
 import numpy as np
 import pytest
@@ -14,8 +15,9 @@ TOL = 1.5e-2
 
 
 def _check(sh, n_samples):
-    from _decoder_harness import Decoder
+    from paper_2607_04068_b200.decoder_harness import Decoder
     from oracle.replay import replay_beam_attention
+    from oracle.tree import sequence_expanded_attention
     from oracle.selection import select_beams
     torch.manual_seed(0)
     model = Decoder(sh, seed=0)
@@ -53,14 +55,27 @@ def _check(sh, n_samples):
         got = cap["out"][t][li][u, i].float().cpu().numpy()
         worst = max(worst, float(np.abs(got - ref).max() / (np.abs(ref).max() + 1e-30)))
     assert worst <= TOL, f"sampled attention rows vs oracle: {worst:.3e}"
+    # (d) ALL beams of whole (layer, user) pairs, every step: first layer / first user and last layer / last user
+    for li, u in ((0, 0), (sh.n_layers - 1, sh.B - 1)):
+        Kp, Vp = cap["prefix_kv"][li]
+        Kp = Kp[u * sh.prefix:(u + 1) * sh.prefix].float().cpu().numpy()
+        Vp = Vp[u * sh.prefix:(u + 1) * sh.prefix].float().cpu().numpy()
+        for t in range(sh.d):
+            k_lv = [cap["k"][l][li][u].float().cpu().numpy() for l in range(1, t + 1)]
+            v_lv = [cap["v"][l][li][u].float().cpu().numpy() for l in range(1, t + 1)]
+            parents = [sel[l][1][u] for l in range(t)]
+            ref = sequence_expanded_attention(Kp, Vp, k_lv, v_lv, parents, cap["q"][t][li][u].float().cpu().numpy(), t, scale)
+            got = cap["out"][t][li][u].float().cpu().numpy()
+            err = float(np.abs(got - ref).max() / (np.abs(ref).max() + 1e-30))
+            assert err <= TOL, f"layer {li} user {u} step {t}: all beams vs oracle {err:.3e}"
 
 
 def test_small_decoder():
-    from _decoder_harness import DecoderShape
+    from paper_2607_04068_b200.decoder_harness import DecoderShape
     _check(DecoderShape(n_layers=3, d_model=256, Hq=8, Hkv=2, D=64, ffn=512, vocab=1000, prefix=300, B=3, W=24, d=3, C=40),
            n_samples=12)
 
 
 def test_cfg3_full_size():
-    from _decoder_harness import DecoderShape
+    from paper_2607_04068_b200.decoder_harness import DecoderShape
     _check(DecoderShape(), n_samples=10)

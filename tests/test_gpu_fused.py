@@ -2,7 +2,8 @@
 kernel: cluster sizes 1/2/4/8 over the prefix splits (DSMEM exchange), splits that are EMPTY for short users
 of a ragged batch, parity mode vs pair mode, a second Q tile with few live rows, head_dim 64, GQA groups of 1,
 2, 4 and 8, chain lengths 0..d.  Reference: oracle.replay (conventional per-beam full-sequence attention,
-fp64) on sampled beams, plus the two-call GPU path (A1 then A2) on every row.  Tolerance: DESIGN.md R20."""
+fp64) -- every row of every user via the sequence-expanded Eq.-14 form, sampled beams via the per-beam
+replay -- plus the two-call GPU path (A1 then A2) on every row.  Tolerance: DESIGN.md R20."""
 import numpy as np
 import pytest
 
@@ -20,6 +21,7 @@ def _bf16(x):
 def _case(B, Hq, Hkv, D, lens, W, d, seed):
     import torch
     from oracle.replay import replay_beam_attention
+    from oracle.tree import sequence_expanded_attention
     from paper_2607_04068_b200.decode import StarkLayer
     rng = np.random.default_rng([0, 91, seed])
     lens = np.asarray(lens)
@@ -57,14 +59,20 @@ def _case(B, Hq, Hkv, D, lens, W, d, seed):
         # every row: fused vs two-call (both bf16 outputs of the same fp32-accumulated math)
         ref_max = np.abs(two).max() + 1e-30
         assert np.abs(fused - two).max() <= TOL * ref_max, f"step {t}: fused vs two-call {np.abs(fused - two).max() / ref_max:.3e}"
-        # sampled beams: fused vs the conventional fp64 oracle
+        # EVERY row of EVERY user: fused vs the fp64 oracle (sequence-expanded masked attention, Eq. 14;
+        # pinned equal to the conventional per-beam form in tests/test_oracle_beam_search.py)
         worst = 0.0
-        for _ in range(6):
+        for u in range(B):
+            ref = sequence_expanded_attention(K[cu[u]:cu[u + 1]], V[cu[u]:cu[u + 1]], [x[u] for x in k_lv[:t]],
+                                              [x[u] for x in v_lv[:t]], [p[u] for p in parents[:t]], q[u], t, scale)
+            worst = max(worst, float(np.abs(fused[u] - ref).max() / (np.abs(ref).max() + 1e-30)))
+        assert worst <= TOL, f"step {t}: fused vs oracle {worst:.3e}"
+        # and the conventional per-beam replay (replicated caches) on sampled beams
+        for _ in range(3):
             u, i = int(rng.integers(B)), int(rng.integers(n_q))
             ref = replay_beam_attention(K[cu[u]:cu[u + 1]], V[cu[u]:cu[u + 1]], [x[u] for x in k_lv[:t]],
                                         [x[u] for x in v_lv[:t]], [p[u] for p in parents[:t]], q[u, i], i, t, scale)
-            worst = max(worst, float(np.abs(fused[u, i] - ref).max() / (np.abs(ref).max() + 1e-30)))
-        assert worst <= TOL, f"step {t}: fused vs oracle {worst:.3e}"
+            assert float(np.abs(fused[u, i] - ref).max() / (np.abs(ref).max() + 1e-30)) <= TOL, f"step {t}: beam ({u},{i})"
 
 
 @pytest.mark.parametrize("name,args", [

@@ -135,3 +135,51 @@ def test_mid_single_cta_path():
     _check(z, np.zeros((2, 32), np.float32), 256)
     w = r.normal(-4, 1, (1, 40, 400)).astype(np.float32); w[0, :, 5:] = -np.inf; w[0, 39, 399] = 3.0
     _check(w, r.normal(0, 1, (1, 40)).astype(np.float32), 256)   # 201 finite keys + 55 of the -inf ties
+
+
+@pytest.mark.parametrize("W_out", [1025, 1536, 2048, 3000])
+@pytest.mark.parametrize("B,W_in,C", [(2, 64, 1024), (1, 512, 1024), (1, 128, 8192), (3, 40, 1000)])
+def test_wide_outputs_above_1024(B, W_in, C, W_out):
+    """1024 < W_out <= 4096 at N >= 32768 (the shared-memory sizing of the pruned cluster kernel):
+    random keys with sorted parent scores, and a tie-heavy 1/4 grid."""
+    r = _rng(8)
+    logits = r.normal(0, 2, (B, W_in, C))
+    logp = (logits - np.log(np.exp(logits).sum(-1, keepdims=True))).astype(np.float32)
+    score = np.sort(r.normal(-8, 2, (B, W_in)).astype(np.float32))[:, ::-1].copy()
+    _check(logp, score, W_out)
+    _check((np.round(logp * 4) / 4).astype(np.float32), (np.round(score * 4) / 4).astype(np.float32), W_out)
+
+
+def test_cfg4_full_size_exact_tie_variant():
+    """"plus an extra exact-tie variant (logits rounded to 1/8) for parity
+    only" at FULL size (8 users x 512 beams x 1024 codes, W_out = 512), every level, all users, through both
+    entries (log-probs and raw logits).  The tree is the oracle's (scores of level t come from its selection of
+    level t-1), so every level is checked on its own."""
+    import torch
+    import workloads as wl
+    from oracle.selection import log_softmax_fp32, select_beams, select_beams_from_logits
+    from paper_2607_04068_b200.decode import beam_topk, beam_topk_logits
+    cfg = wl.get_config("cfg4")
+    nq, widths = wl.queries_per_step(cfg), wl.beam_widths(cfg)
+    for from_logits in (False, True):
+        score = None
+        for t in range(cfg.d):
+            lg = wl.tie_logits(wl.step_logits(cfg, t, nq[t]))
+            assert np.array_equal(lg * 8, np.round(lg * 8))
+            x = lg if from_logits else log_softmax_fp32(lg)
+            sc = None if score is None else torch.from_numpy(score).cuda()
+            fn = beam_topk_logits if from_logits else beam_topk
+            s_g, p_g, c_g = [a.cpu().numpy() for a in fn(torch.from_numpy(x).cuda(), sc, widths[t])]
+            nxt = []
+            for u in range(cfg.B):
+                s_u = np.zeros(nq[t], np.float32) if score is None else score[u]
+                s_r, p_r, c_r = (select_beams_from_logits if from_logits else select_beams)(s_u, x[u], widths[t])
+                assert np.array_equal(p_g[u], p_r) and np.array_equal(c_g[u], c_r), f"level {t} user {u} ({from_logits=})"
+                assert np.array_equal(s_g[u].view(np.uint32), s_r.view(np.uint32)), f"level {t} user {u} score bits"
+                nxt.append(s_r)
+            score = np.stack(nxt)
+    # the same shape with keys on an exact grid ACROSS beams (log-probs and scores both multiples of 1/8)
+    r = _rng(9)
+    logp = (np.round(r.normal(-7, 1.5, (cfg.B, 512, cfg.C)) * 8) / 8).astype(np.float32)
+    score = np.sort((np.round(r.normal(-5, 1, (cfg.B, 512)) * 8) / 8).astype(np.float32))[:, ::-1].copy()
+    _check(logp, score, 512)
