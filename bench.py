@@ -1,13 +1,19 @@
 #!/usr/bin/env python
 """bench.py -- STARK decode hot path on B200 (contract: see DESIGN.md section 7).
 
-A "step" = one whole pass of the hot path over one batch of
-BASELINE.json configs[1] ("cfg2"): decode steps t = 0,1,2, each
+A "step" = one whole pass of the hot path over one batch of the workload:
+decode steps t = 0..d-1, each
     bf16: stark_decode_step (A4 + A1 + A2 in one launch) -> stark_beam_topk
     fp32: stark_kv_append_reorg (t>=1) -> stark_prefix_attn -> stark_tree_attn_step -> stark_beam_topk.
 metric = generated SIDs/s (B * W_d final beams per pass / pass time); also us per decode step.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl stark|reference] [--workload cfg2]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl stark|reference] [--workload cfg5]
+
+Headline workload: cfg5 (BASELINE.json configs[4], the largest single-GPU configuration; BASELINE.json's metric
+names no configuration).  The same JSON line carries `per_config`: cfg1, cfg2, cfg3 (attention-side shape), cfg4,
+paper_b8, paper_b1 -- pass time (median and min over >= 100 graph replays), SIDs/s and a per-kernel table (fused
+launches AND the four north-star calls as separate launches) with roofline fractions against the measured and
+the nominal peaks.
 
 N > 1 (torchrun): users are independent, so every rank runs its own batch (weak scaling, no data-path
 collective); time = max over ranks.  --impl reference times the CPU oracle (oracle/) on a bounded sample.
@@ -17,6 +23,7 @@ from __future__ import annotations
 import argparse
 import json
 import os
+import subprocess
 import sys
 import threading
 import time
@@ -31,15 +38,20 @@ import workloads as wl  # noqa: E402
 METRIC, UNIT = "generated SIDs/s (tree-attn decode, all steps)", "SIDs/s"
 L2_BYTES = 126 * 2 ** 20
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+NOMINAL = {"hbm_gbs": 8000.0, "bf16_tflops": 2250.0}     # north star "~8 TB/s"; vendor dense bf16
+HEADLINE = "cfg5"
+PER_CONFIG = ["cfg1", "cfg2", "cfg3", "cfg4", "paper_b8", "paper_b1"]
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=2000)
-    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="stark", choices=["stark", "reference"])
-    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--workload", default=HEADLINE)
+    ap.add_argument("--per-config", default=",".join(PER_CONFIG),
+                    help="comma-separated workloads measured into `per_config` (rank 0, N = 1 only); '' = none")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--from-logits", action="store_true",
                     help="selection consumes RAW logits (stark_beam_topk_logits, SURVEY 8f-1) instead of log-probs")
@@ -47,6 +59,9 @@ def parse_args():
     ap.add_argument("--sets", type=int, default=0, help="rotating input sets (0 = enough to exceed L2)")
     ap.add_argument("--calibrate", action="store_true",
                     help="print launch-floor / cold-stream floors of this GPU (DESIGN.md section 7) and exit")
+    ap.add_argument("--traffic-from", default=None, metavar="NCU_RAW_CSV",
+                    help="update profiles/traffic.json for --workload from `ncu -i x.ncu-rep --page raw --csv` output "
+                         "(dram__bytes_read.sum + dram__bytes_write.sum per launch) and exit")
     return ap.parse_args()
 
 
@@ -56,6 +71,26 @@ def peaks():
         d = json.load(open(p))
         return {k: float(d[k]) for k in FALLBACK_PEAKS if k in d} | {"source": "measured"}
     return dict(FALLBACK_PEAKS) | {"source": "fallback"}
+
+
+def git_head():
+    try:
+        return subprocess.run(["git", "-C", ROOT, "rev-parse", "--short=12", "HEAD"], capture_output=True,
+                              text=True, timeout=10).stdout.strip() or None
+    except Exception:  # noqa: BLE001
+        return None
+
+
+def cpu_info():
+    model = None
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                model = ln.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"model": model, "logical_cpus": os.cpu_count()}
 
 
 # ------------------------------------------------------------------------------------------
@@ -100,6 +135,8 @@ def host_inputs(cfg, seed):
     for t in range(cfg.d):
         qq, kk, vv = wl.step_qkv(cfg, t, nq[t], seed)
         q.append(qq), k.append(kk), v.append(vv)
+        # (config 1 derives its logits from the attention output when it runs free, tests/test_gpu_e2e_cfg1.py; a
+        # timed pass needs fixed inputs, so there wl.step_logits' seeded N(0, 2) draws of the same shape stand in)
         lg.append(wl.step_logits(cfg, t, nq[t], seed))
     return dict(K=K, V=V, cu=cu, q=q, k=k, v=v, lg=lg)
 
@@ -157,14 +194,33 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons), "samples": len(s)}
 
 
-def time_graph_loop(torch, fns, iters, use_graph=True):
-    """Average device time (us) of one call of each fn in `fns` (one per rotating input set, so that
-    consecutive launches never find their inputs in L2).  All of them are captured, round-robin, into ONE
-    CUDA graph that is replayed; CUDA events on the launching stream bracket the replays.  (One graph per
-    launch would measure the graph-launch cadence instead: back-to-back single-kernel graphs start on a
-    ~2.05 us grid on this machine, see profiles/r01b_calibration.md.)"""
+def replay_stats(torch, call, units_per_call, replays):
+    """CUDA events on the launching stream around EACH of `replays` calls (after 3 warm-up calls); returns
+    (median, min, mean) device time in us per unit (a call holds `units_per_call` passes or launches)."""
+    for _ in range(3):
+        call()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(replays)]
+    torch.cuda.synchronize()
+    for a, b in ev:
+        a.record()
+        call()
+        b.record()
+    torch.cuda.synchronize()
+    us = np.array([a.elapsed_time(b) for a, b in ev]) * 1e3 / units_per_call
+    return float(np.median(us)), float(us.min()), float(us.mean())
+
+
+def time_graph_loop(torch, fns, iters, use_graph=True, stats=False):
+    """Device time (us) of one call of each fn in `fns` (one per rotating input set, so that consecutive launches
+    never find their inputs in L2).  All of them are captured, round-robin, into ONE CUDA graph that is replayed;
+    CUDA events on the launching stream bracket every replay.  (One graph per launch would measure the
+    graph-launch cadence instead: back-to-back single-kernel graphs start on a ~2.05 us grid on this machine,
+    see profiles/r01b_calibration.md.)  Returns the median over replays (stats=True: (median, min))."""
     per_graph = max(len(fns), 24 // len(fns) * len(fns))
-    reps = max(1, iters // per_graph)
+    reps = max(5, iters // per_graph)
+    for f in fns:                          # eager first call: lazy buffers and function attributes, outside the capture
+        f()
+    torch.cuda.synchronize()
     if use_graph:
         g = torch.cuda.CUDAGraph()
         with torch.cuda.graph(g):
@@ -175,47 +231,92 @@ def time_graph_loop(torch, fns, iters, use_graph=True):
         def call():
             for i in range(per_graph):
                 fns[i % len(fns)]()
-    for _ in range(3):
-        call()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    e0.record()
-    for _ in range(reps):
-        call()
-    e1.record()
-    torch.cuda.synchronize()
-    return e0.elapsed_time(e1) * 1e3 / (reps * per_graph)
+    med, mn, _ = replay_stats(torch, call, per_graph, reps)
+    return (med, mn) if stats else med
 
 
 # ------------------------------------------------------------------------------------------
-def oracle_sample(cfg, n_users, seed=0):
-    """The CPU oracle (conventional fp64 beam search, oracle/) as it stands on `n_users` users of the
-    workload.  Returns (seconds, SIDs generated, threads used)."""
+def _oracle_user(job):
+    """One user of the workload through the oracle as it stands (worker of the process pool)."""
+    name, u, seed = job
     from oracle.beam_search import conventional_beam_search
     from oracle.token_models import DrawTokenModel
-    users = list(range(n_users))
+    cfg = wl.get_config(name)
     lens = wl.prefix_lengths(cfg, seed)
     nq = wl.queries_per_step(cfg)
-    per_user = []
-    for u in users:
-        K, V = wl.prefix_kv_user(cfg, u, int(lens[u]), seed)
-        q, k, v, lg = [], [], [], []
-        for t in range(cfg.d):
-            qq, kk, vv = wl.step_qkv(cfg, t, nq[t], seed, users=[u])
-            q.append(qq[0]), k.append(kk[0]), v.append(vv[0])
-            lg.append(wl.step_logits(cfg, t, nq[t], seed, users=[u])[0])
-        per_user.append((K, V, DrawTokenModel(q, k, v, lg)))
-    try:
-        from threadpoolctl import threadpool_info
-        threads = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
-    except Exception:  # noqa: BLE001
-        threads = 1
+    K, V = wl.prefix_kv_user(cfg, u, int(lens[u]), seed)
+    q, k, v, lg = [], [], [], []
+    for t in range(cfg.d):
+        qq, kk, vv = wl.step_qkv(cfg, t, nq[t], seed, users=[u])
+        q.append(qq[0]), k.append(kk[0]), v.append(vv[0])
+        lg.append(wl.step_logits(cfg, t, nq[t], seed, users=[u])[0])
     t0 = time.perf_counter()
-    n_sids = 0
-    for K, V, m in per_user:
-        tr = conventional_beam_search(K, V, m, cfg.W, cfg.C, 1.0 / np.sqrt(cfg.D))
-        n_sids += tr.paths.shape[0]
-    return time.perf_counter() - t0, n_sids, threads
+    tr = conventional_beam_search(K, V, DrawTokenModel(q, k, v, lg), cfg.W, cfg.C, 1.0 / np.sqrt(cfg.D))
+    return time.perf_counter() - t0, int(tr.paths.shape[0])
+
+
+def _noop(_):
+    return 0
+
+
+def oracle_sample_users(cfg, seed=0):
+    """The bounded sample of the workload the oracle is timed on: users in order of increasing prefix length,
+    as many as fit ~20 s of CPU work and the host's memory (the oracle replicates every beam's whole KV cache:
+    W * L * Hkv * D * 16 B per user)."""
+    lens = wl.prefix_lengths(cfg, seed)
+    order = np.argsort(lens, kind="stable")
+    W = max(wl.beam_widths(cfg))
+    try:
+        import psutil
+        avail_gb = psutil.virtual_memory().available / 2 ** 30
+    except Exception:  # noqa: BLE001
+        avail_gb = 16.0
+    budget_users = {"cfg1": 1, "cfg2": 8, "cfg3": 2, "cfg4": 2, "cfg5": 2}.get(cfg.name, 1)
+    users, mem = [], 0.0
+    for u in order[:min(budget_users, cfg.B, os.cpu_count() or 1)]:
+        g = W * int(lens[u]) * cfg.Hkv * cfg.D * 16 / 2 ** 30
+        if users and mem + g > 0.4 * avail_gb:
+            break
+        users.append(int(u))
+        mem += g
+    return users, lens
+
+
+def oracle_sample(cfg, users, seed=0):
+    """The CPU oracle (conventional fp64 beam search, oracle/) as it stands on `users` of the workload, one
+    process per user (users are independent; BLAS threads pinned to 1 per process so that `cores` is what was
+    used).  Returns (wall seconds, SIDs generated, cores used)."""
+    import multiprocessing as mp
+    jobs = [(cfg.name, u, seed) for u in users]
+    n_proc = max(1, min(len(users), os.cpu_count() or 1))
+    if n_proc == 1:
+        try:
+            from threadpoolctl import threadpool_limits
+            with threadpool_limits(limits=1):
+                t0 = time.perf_counter()
+                res = [_oracle_user(j) for j in jobs]
+                wall = time.perf_counter() - t0
+        except ImportError:
+            t0 = time.perf_counter()
+            res = [_oracle_user(j) for j in jobs]
+            wall = time.perf_counter() - t0
+        return wall, sum(r[1] for r in res), 1
+    keys = ("OMP_NUM_THREADS", "OPENBLAS_NUM_THREADS", "MKL_NUM_THREADS")
+    saved = {k: os.environ.get(k) for k in keys}
+    os.environ.update({k: "1" for k in keys})           # inherited by the workers (spawned: a fresh numpy)
+    try:
+        with mp.get_context("spawn").Pool(n_proc) as pool:
+            pool.map(_noop, range(n_proc))               # workers up and modules imported: not timed
+            t0 = time.perf_counter()
+            res = pool.map(_oracle_user, jobs, chunksize=1)
+            wall = time.perf_counter() - t0
+    finally:
+        for k, v in saved.items():
+            if v is None:
+                os.environ.pop(k, None)
+            else:
+                os.environ[k] = v
+    return wall, sum(r[1] for r in res), n_proc
 
 
 def shard_seed(rank: int, r: int) -> int:
@@ -258,10 +359,42 @@ def run_calibrate():
     print(json.dumps({"calibration": out}), flush=True)
 
 
+def run_traffic_from(args):
+    """profiles/traffic.json[workload][kernel.tN] = DRAM bytes of that launch, from the raw-page CSV of an
+    `ncu --set full` capture of `python bench.py --workload W --no-cpu-baseline --per-config '' ...`: the k-th
+    captured launch of a kernel family is matched to decode step t by launch order (one pass = d steps, each
+    decode attention then top-k)."""
+    import csv
+    rows = list(csv.DictReader(open(args.traffic_from)))
+    cfg = wl.get_config(args.workload)
+    fam = {"prefix_tc_kernel": "decode_step", "topk": "beam_topk"}
+    seen, out = {}, {}
+    for r in rows:
+        name = r.get("Kernel Name", "")
+        key = next((v for k, v in fam.items() if k in name), None)
+        if key is None:
+            continue
+        try:
+            byts = float(r["dram__bytes_read.sum"].replace(",", "")) + float(r["dram__bytes_write.sum"].replace(",", ""))
+        except (KeyError, ValueError):
+            continue                                     # (the units row)
+        t = seen.get(key, 0)
+        seen[key] = t + 1
+        if t < cfg.d:
+            out[f"{key}.t{t}"] = int(byts)
+    units = next((r.get("dram__bytes_read.sum") for r in rows if not r.get("Kernel Name")), None)
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    allj = json.load(open(tpath)) if os.path.exists(tpath) else {}
+    allj[cfg.name] = out | {"_source": {"csv": os.path.relpath(os.path.abspath(args.traffic_from), ROOT),
+                                        "unit": units, "head": git_head(), "date": time.strftime("%Y-%m-%d")}}
+    json.dump(allj, open(tpath, "w"), indent=1)
+    print(json.dumps({cfg.name: allj[cfg.name]}))
+
+
 def run_cfg3_decoder(args):
-    """BASELINE configs[2]: the library inside a 12-layer random-init decoder (paper_2607_04068_b200/decoder_harness.py; GEMMs in
-    torch/cuBLAS, not graded).  Prefill untimed.  Reports the whole decode (4 levels x 12 layers) and the
-    library calls alone (same captured inputs, no GEMMs), eager launches, CUDA events."""
+    """BASELINE configs[2]: the library inside a 12-layer random-init decoder
+    (paper_2607_04068_b200/decoder_harness.py; GEMMs in torch/cuBLAS, not graded).  Prefill untimed.  Reports the
+    whole decode (4 levels x 12 layers) and the library calls alone (same captured inputs, no GEMMs)."""
     import torch
     from paper_2607_04068_b200.decoder_harness import Decoder, DecoderShape
     sh = DecoderShape()
@@ -314,42 +447,169 @@ def run_cfg3_decoder(args):
 
 
 def run_reference(args, cfg):
+    """The reference arm of this tier = the oracle as it stands on the box's host cores (rank 0 only): each step
+    one bounded sample of the workload (the users oracle_sample_users picks), ~2.5 minutes at most in total."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n_users = 1
-    lens = wl.prefix_lengths(cfg, 0)
-    for _ in range(args.warmup):
-        pass  # the oracle has no warm-up state; nothing to do
-    steps = max(1, min(args.steps, 5))
-    times, sids = [], 0
-    threads = 1
-    for _ in range(steps):
-        dt, n, threads = oracle_sample(cfg, n_users)
+    users, lens = oracle_sample_users(cfg)
+    times, sids, procs = [], 0, 1
+    t_start = time.perf_counter()
+    for _ in range(max(1, args.steps)):
+        dt, n, procs = oracle_sample(cfg, users)
         times.append(dt)
         sids += n
+        if time.perf_counter() - t_start + dt > 150.0:     # the next step would overrun the budget
+            break
+    steps = len(times)
     total = float(np.sum(times))
     val = sids / total
+    sample = (f"users {users} of {cfg.B} (prefix lengths {[int(lens[u]) for u in users]}) per step, all {cfg.d} decode "
+              f"steps, one process per user")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * total / steps * cfg.B / n_users, "higher_is_better": True,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / steps * cfg.B / len(users), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "B": cfg.B, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D,
                        "prefix_len": [int(lens.min()), int(lens.max())], "beam": list(wl.beam_widths(cfg)),
-                       "levels": cfg.d, "codebook": cfg.C, "decode_steps_per_pass": cfg.d,
-                       "sample": f"{n_users} of {cfg.B} users per step, all {cfg.d} decode steps"},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle",
-                             "sample": f"{n_users} of {cfg.B} users x {steps} repeats"},
+                       "levels": cfg.d, "codebook": cfg.C, "decode_steps_per_pass": cfg.d, "sample": sample,
+                       "ms_per_step_note": f"extrapolated x B / n_users = x {cfg.B}/{len(users)} from the timed sample "
+                                           f"({1e3 * total / steps:.0f} ms per timed step); {steps} of the requested "
+                                           f"{args.steps} steps fit the 150 s budget"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": procs, "kind": "oracle",
+                             "sample": f"{sample} x {steps} repeats", "cpu": cpu_info()},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
 
 
 # ------------------------------------------------------------------------------------------
+def build_sets(cfg, rank, dev, from_logits, n_sets):
+    """R rotating input sets (host + device) so that consecutive passes never hit a warm L2."""
+    h0 = host_inputs(cfg, seed=shard_seed(rank, 0))
+    eb = cfg.elem_bytes
+    set_bytes = sum(a.size * eb for a in [h0["K"], h0["V"], *h0["q"], *h0["k"], *h0["v"]]) + sum(a.nbytes for a in h0["lg"])
+    R = n_sets or int(min(16, max(2, -(-2 * L2_BYTES // set_bytes))))
+    hosts = [h0] + [host_inputs(cfg, seed=shard_seed(rank, r)) for r in range(1, R)]
+    passes = [make_pass(cfg, h, dev, from_logits=from_logits) for h in hosts]
+    return hosts, passes, R, set_bytes
+
+
+def capture_passes(torch, passes, use_graph):
+    """(calls: one replayable pass per input set; call_all: ONE graph holding a pass over each of the R sets)."""
+    for p in passes:                       # eager warm-up: function attributes, lazy module load
+        p.run()
+    torch.cuda.synchronize()
+    if not use_graph:
+        def call_all():
+            for p in passes:
+                p.run()
+        return [p.run for p in passes], call_all
+    calls = []
+    for p in passes:
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            p.run()
+        calls.append(g.replay)
+    # graph-to-graph hand-over costs ~1 us of idle GPU per replay: paid once per R passes
+    g_all = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g_all):
+        for p in passes:
+            p.run()
+    return calls, g_all.replay
+
+
+def kernel_table(torch, cfg, passes, lens, pk, use_graph, from_logits, two_call=True, iters=240):
+    """Per-kernel device times over the rotating sets (CUDA events around graph replays; median and min over the
+    replays) with the algorithmic bytes / FLOPs of one launch and the roofline fractions
+    against the measured (MEASURED_PEAKS.json) and the nominal (8 TB/s, 2.25 PFLOP/s) peaks.  Entries: the
+    launches of the timed pass, and (two_call) the four north-star calls as separate launches."""
+    nq, widths = wl.queries_per_step(cfg), wl.beam_widths(cfg)
+    p0 = passes[0]
+    kern = {}
+
+    def put(name, fns, byts, flops=None, **extra):
+        med, mn = time_graph_loop(torch, fns, iters, use_graph, stats=True)
+        kern[name] = {"us": med, "us_min": mn, "bytes": byts} | ({"flops": flops} if flops is not None else {}) | extra
+
+    for t in range(cfg.d):
+        if p0.inline_append:      # stark_decode_step: the level's append rides inside the attention launch
+            fl, by = work_decode(cfg, lens, nq[t], t)
+            if t >= 1:
+                by += work_append(cfg, nq[t])
+            put(f"decode_step.t{t}", [(lambda p=p, t=t: p.layer.step(t, p.q[t], p.k_new[t] if t else None,
+                                                                     p.v_new[t] if t else None,
+                                                                     p.sel[t - 1][1] if t else None, out=p.out[t]))
+                                      for p in passes], by, fl)
+        put(("beam_topk_logits" if from_logits else "beam_topk") + f".t{t}",
+            [(lambda p=p, t=t: p.select(t, p.sel[t - 1][0] if t else None)) for p in passes],
+            work_topk(cfg, nq[t], widths[t]))
+        if two_call or not p0.inline_append:
+            ns = p0.layer.n_splits(nq[t])
+            fl, by = work_prefix(cfg, lens, nq[t], ns)
+            put(f"prefix_attn.t{t}", [(lambda p=p, t=t: p.layer.prefix(p.q[t])) for p in passes], by, fl, n_splits=ns)
+            put(f"tree_attn_step.t{t}", [(lambda p=p, t=t: p.layer.tree(t, p.q[t], p.out[t])) for p in passes],
+                work_tree(cfg, nq[t], t, ns))
+            if t >= 1:
+                put(f"kv_append_reorg.t{t}", [(lambda p=p, t=t: p.layer.append(t, p.k_new[t], p.v_new[t], p.sel[t - 1][1]))
+                                              for p in passes], work_append(cfg, nq[t]))
+    hbm, tfl = pk["hbm_gbs"], pk["bf16_tflops"]
+    for v in kern.values():
+        v["GBps"] = v["bytes"] / v["us"] * 1e-3
+        fl = v.get("flops", 0.0) if cfg.dtype == "bf16" else 0.0
+        t_h, t_t = v["bytes"] / (hbm * 1e3), fl / (tfl * 1e6)                       # us
+        v["roofline_us"] = max(t_h, t_t)
+        v["bound"] = "tensor" if t_t > t_h else "hbm"
+        v["frac"] = v["roofline_us"] / v["us"]
+        v["frac_nominal"] = max(v["bytes"] / (NOMINAL["hbm_gbs"] * 1e3), fl / (NOMINAL["bf16_tflops"] * 1e6)) / v["us"]
+    return kern
+
+
+def in_pass(name, p0):
+    """Is this kernel-table entry one of the launches of the timed pass?"""
+    fam = name.split(".")[0]
+    if p0.inline_append:
+        return fam in ("decode_step", "beam_topk", "beam_topk_logits")
+    return fam in ("prefix_attn", "tree_attn_step", "kv_append_reorg", "beam_topk", "beam_topk_logits")
+
+
+def rnd(d):
+    return {k: ({a: (round(b, 4) if isinstance(b, float) else b) for a, b in v.items()} if isinstance(v, dict) else v)
+            for k, v in d.items()}
+
+
+def measure_config(torch, cfg, dev, pk, args, replays=100):
+    """One `per_config` entry: pass time (median / min over `replays` replays of the R-pass graph), SIDs/s,
+    per-kernel table."""
+    t_in = time.perf_counter()
+    hosts, passes, R, set_bytes = build_sets(cfg, 0, dev, args.from_logits, args.sets)
+    use_graph = not args.no_graph
+    calls, call_all = capture_passes(torch, passes, use_graph)
+    med, mn, mean = replay_stats(torch, call_all, R, replays)
+    lens = np.diff(hosts[0]["cu"])
+    widths = wl.beam_widths(cfg)
+    kern = kernel_table(torch, cfg, passes, lens, pk, use_graph, args.from_logits)
+    sids = cfg.B * widths[-1]
+    ent = {"pass_us_median": med, "pass_us_min": mn, "pass_us_mean": mean, "replays": replays,
+           "passes_per_replay": R, "sids_per_s": sids / (med * 1e-6), "us_per_decode_step": med / cfg.d,
+           "launches_per_pass": passes[0].launches, "dtype": cfg.dtype,
+           "shape": {"B": cfg.B, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D, "prefix_len": [int(lens.min()), int(lens.max())],
+                     "beam": list(widths), "levels": cfg.d, "codebook": cfg.C},
+           "l2": f"{R} rotating input sets ({R * set_bytes / 2**20:.0f} MiB)",
+           "kernel_sum_us": sum(v["us"] for k, v in kern.items() if in_pass(k, passes[0])),
+           "kernels": rnd(kern)}
+    if cfg.name == "cfg1" and not args.no_cpu_baseline:
+        sec, n, procs = oracle_sample(cfg, [0])
+        ent["cpu_oracle"] = {"pass_us": sec * 1e6, "sids_per_s": n / sec, "cores": procs}
+    del hosts, passes, calls, call_all
+    torch.cuda.empty_cache()
+    ent["bench_wall_s"] = round(time.perf_counter() - t_in, 1)
+    return ent
+
+
 def run_stark(args, cfg):
     import torch
     import torch.distributed as dist
     from paper_2607_04068_b200.build import build
     from paper_2607_04068_b200 import binding as sb
-    from paper_2607_04068_b200.decode import beam_topk
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -367,42 +627,14 @@ def run_stark(args, cfg):
     sb.lib()
 
     # ---- inputs: R rotating sets so that consecutive passes never hit a warm L2 ----------------
-    h0 = host_inputs(cfg, seed=shard_seed(rank, 0))
-    set_bytes = sum(a.nbytes // (2 if cfg.dtype == "bf16" else 1) for a in [h0["K"], h0["V"], *h0["q"], *h0["k"], *h0["v"]]) \
-        + sum(a.nbytes for a in h0["lg"])
-    R = args.sets or int(min(16, max(2, -(-2 * L2_BYTES // set_bytes))))
-    hosts = [h0] + [host_inputs(cfg, seed=shard_seed(rank, r)) for r in range(1, R)]
-    passes = [make_pass(cfg, h, dev, from_logits=args.from_logits) for h in hosts]
+    hosts, passes, R, set_bytes = build_sets(cfg, rank, dev, args.from_logits, args.sets)
+    h0 = hosts[0]
     lens = np.diff(h0["cu"])
     widths = wl.beam_widths(cfg)
-    nq = wl.queries_per_step(cfg)
     sids_per_pass = cfg.B * widths[-1]
     launches_per_pass = passes[0].launches
-
-    for p in passes:                       # eager warm-up: function attributes, lazy module load
-        p.run()
-    torch.cuda.synchronize()
     use_graph = not args.no_graph
-    if use_graph:
-        calls = []
-        for p in passes:
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g):
-                p.run()
-            calls.append(g.replay)
-        # the timed loop replays ONE graph holding a pass over each of the R input sets (graph-to-graph hand-over
-        # costs ~1 us of idle GPU per replay: paid once per R passes); a remainder of K mod R uses the single graphs
-        g_all = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(g_all):
-            for p in passes:
-                p.run()
-        call_all = g_all.replay
-    else:
-        calls = [p.run for p in passes]
-
-        def call_all():
-            for p in passes:
-                p.run()
+    calls, call_all = capture_passes(torch, passes, use_graph)
 
     def run_steps(n):          # exactly n passes
         for _ in range(n // R):
@@ -448,61 +680,29 @@ def run_stark(args, cfg):
             dist.destroy_process_group()
         return
 
-    # ---- per-kernel device times (graphs of single launches over the rotating sets) -------------
+    # ---- pass statistics + per-kernel device times (graphs over the rotating sets) -------------
     pk = peaks()
-    kern = {}
-    it = 40 * R
-    for t in range(cfg.d):
-        if passes[0].inline_append:      # stark_decode_step: the level's append rides inside the attention launch
-            fl, by = work_decode(cfg, lens, nq[t], t)
-            if t >= 1:
-                by += work_append(cfg, nq[t])
-            us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.step(t, p.q[t], p.k_new[t] if t else None,
-                                                                        p.v_new[t] if t else None,
-                                                                        p.sel[t - 1][1] if t else None, out=p.out[t]))
-                                         for p in passes], it, use_graph)
-            kern[f"decode_step.t{t}"] = {"us": us, "bytes": by, "flops": fl}
-        elif passes[0].fused:
-            fl, by = work_decode(cfg, lens, nq[t], t)
-            us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.attend(t, p.q[t], out=p.out[t], fused=True))
-                                         for p in passes], it, use_graph)
-            kern[f"decode_attn.t{t}"] = {"us": us, "bytes": by, "flops": fl}
-        else:
-            ns = passes[0].layer.n_splits(nq[t])
-            fl, by = work_prefix(cfg, lens, nq[t], ns)
-            us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.prefix(p.q[t])) for p in passes], it, use_graph)
-            kern[f"prefix_attn.t{t}"] = {"us": us, "bytes": by, "flops": fl, "n_splits": ns}
-            us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.tree(t, p.q[t], p.out[t])) for p in passes], it, use_graph)
-            kern[f"tree_attn_step.t{t}"] = {"us": us, "bytes": work_tree(cfg, nq[t], t, ns)}
-        w_in = nq[t]
-        us = time_graph_loop(torch, [(lambda p=p, t=t: p.select(t, p.sel[t - 1][0] if t else None))
-                                     for p in passes], it, use_graph)
-        kern[("beam_topk_logits" if args.from_logits else "beam_topk") + f".t{t}"] = {
-            "us": us, "bytes": work_topk(cfg, w_in, widths[t])}
-        if t >= 1 and not passes[0].inline_append:
-            us = time_graph_loop(torch, [(lambda p=p, t=t: p.layer.append(t, p.k_new[t], p.v_new[t], p.sel[t - 1][1]))
-                                         for p in passes], it, use_graph)
-            kern[f"kv_append_reorg.t{t}"] = {"us": us, "bytes": work_append(cfg, nq[t])}
+    p_med, p_min, _ = replay_stats(torch, call_all, R, 100 if use_graph else 20)
+    kern = kernel_table(torch, cfg, passes, lens, pk, use_graph, args.from_logits)
     hbm, tfl = pk["hbm_gbs"], pk["bf16_tflops"]
-    for k, v in kern.items():
-        v["GBps"] = v["bytes"] / v["us"] * 1e-3
-        t_h = v["bytes"] / (hbm * 1e3)                       # us
-        t_t = v.get("flops", 0.0) / (tfl * 1e6) if cfg.dtype == "bf16" else 0.0
-        v["roofline_us"] = max(t_h, t_t)
-        v["bound"] = "tensor" if t_t > t_h else "hbm"
-        v["frac"] = v["roofline_us"] / v["us"]
-    ksum = sum(v["us"] for v in kern.values())
-    dom = max(kern, key=lambda k: kern[k]["us"])
+    timed = {k: v for k, v in kern.items() if in_pass(k, passes[0])}
+    ksum = sum(v["us"] for v in timed.values())
+    dom = max(timed, key=lambda k: timed[k]["us"])
     dv = kern[dom]
     if dv["bound"] == "tensor":
         roof = {"bound": "tensor", "achieved": dv["flops"] / dv["us"] * 1e-6, "peak": tfl, "unit": "TFLOP/s"}
+        roof["frac_nominal"] = roof["achieved"] / NOMINAL["bf16_tflops"]
     else:
         roof = {"bound": "hbm", "achieved": dv["GBps"], "peak": hbm, "unit": "GB/s"}
+        roof["frac_nominal"] = roof["achieved"] / NOMINAL["hbm_gbs"]
     roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": None, "kernel": dom,
-                 "kernel_us": dv["us"], "share_of_step": dv["us"] / ksum, "peak_source": pk["source"]})
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # written by hand from an ncu --set full capture
+                 "kernel_us": dv["us"], "share_of_step": dv["us"] / ksum,
+                 "peak_source": pk["source"] + (" (burst figure: the kernel is timed alone)" if dv["bound"] == "tensor" else "")})
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # written by `bench.py --traffic-from <ncu raw csv>`
     if os.path.exists(tpath):
-        roof["traffic"] = json.load(open(tpath)).get(cfg.name, {}).get(dom)
+        tj = json.load(open(tpath)).get(cfg.name, {})
+        roof["traffic"] = tj.get(dom)
+        roof["traffic_source"] = tj.get("_source")
 
     # ---- e2e: HOST buffers in, HOST result out, copies inside the timed region ------------------
     # Two device input sets are used in turn (double buffering): the H2D copy of pass i+1 runs on a copy stream
@@ -521,6 +721,7 @@ def run_stark(args, cfg):
         res_h = [torch.empty(x.shape, dtype=x.dtype).pin_memory() for x in res_d]
         bufs.append((src, dst, res_d, res_h))
     h2d = sum(x.numel() * x.element_size() for x in bufs[0][0])
+    h2d_prefix = sum(x.numel() * x.element_size() for x in bufs[0][0][:2])
     d2h = sum(x.numel() * x.element_size() for x in bufs[0][3])
     s_in, s_run = torch.cuda.Stream(), torch.cuda.Stream()
     ev_in = [torch.cuda.Event() for _ in range(NB)]
@@ -548,6 +749,18 @@ def run_stark(args, cfg):
             ev_out[(i - 1) % NB].synchronize()           # the caller reads pass i-1's result on the host
         ev_out[(n - 1) % NB].synchronize()
 
+    # the prefix upload alone (same pinned buffers, same stream): what share of the e2e pass it is
+    ec0, ec1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(s_in):
+        for rep in range(5):
+            if rep == 1:
+                ec0.record(s_in)
+            for s_, d_ in zip(bufs[0][0][:2], bufs[0][1][:2]):
+                d_.copy_(s_, non_blocking=True)
+        ec1.record(s_in)
+    torch.cuda.synchronize()
+    prefix_ms = ec0.elapsed_time(ec1) / 4
+
     n_e2e = max(4, min(args.steps, 40))
     torch.cuda.synchronize()
     e2e_run(4)
@@ -558,9 +771,14 @@ def run_stark(args, cfg):
     e2e_ms = (time.perf_counter() - t0) * 1e3 / n_e2e
     e2e = {"value": world * sids_per_pass / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": n_e2e,
-           "note": "prefix K/V + per-step q/k/v/log-probs (raw logits with --from-logits) copied from pinned host memory every pass; "
-                   "per-level (score,parent,code) read back; two input sets in turn, the copy of pass i+1 "
-                   "overlaps pass i (wall clock, host waits for every result)"}
+           "prefix_upload_ms": prefix_ms, "prefix_upload_share": prefix_ms / e2e_ms,
+           "h2d_prefix_bytes_per_step": h2d_prefix,
+           "note": "prefix K/V + per-step q/k/v/log-probs (raw logits with --from-logits) copied from pinned host memory "
+                   "every pass; per-level (score,parent,code) read back; two input sets in turn, the copy of pass i+1 "
+                   "overlaps pass i (wall clock, host waits for every result).  PCIe-bound by construction: the "
+                   f"immutable prefix K/V ({h2d_prefix / 2**20:.0f} of the {h2d / 2**20:.0f} MiB) is re-uploaded every pass; "
+                   f"that upload alone takes {prefix_ms:.3f} ms = {100 * prefix_ms / e2e_ms:.0f} % of the {e2e_ms:.3f} ms "
+                   f"e2e pass (device-timed pass: {ms_per_step:.3f} ms)"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -572,16 +790,32 @@ def run_stark(args, cfg):
                        "l2": f"{R} rotating input sets ({R * set_bytes / 2**20:.0f} MiB > L2 126 MiB), no flush",
                        "launch": f"cuda_graph ({R} passes, one per input set, per graph)" if use_graph else "eager"},
             "us_per_decode_step": ms_per_step * 1e3 / cfg.d,
+            "pass_us_median": p_med, "pass_us_min": p_min,
             "gpu_launches": launches_per_pass * args.steps,
             "clocks": sampler.summary(), "e2e": e2e, "roofline": roof,
-            "kernels": {k: {a: (round(b, 4) if isinstance(b, float) else b) for a, b in v.items()} for k, v in kern.items()},
-            "kernel_sum_us": ksum}
+            "peaks": {"measured": dict(pk), "nominal": NOMINAL},
+            "kernels": rnd(kern), "kernel_sum_us": ksum, "head": git_head()}
     if world == 1 and not args.no_cpu_baseline:
-        n_users = 8 if cfg.name == "cfg2" else 1
-        sec, n_sids, threads = oracle_sample(cfg, n_users)
-        line["cpu_baseline"] = {"value": n_sids / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
-                                "sample": f"{n_users} of {cfg.B} users of {cfg.name}, all {cfg.d} decode steps, "
-                                          f"{sec:.1f} s wall"}
+        users, _ = oracle_sample_users(cfg)
+        sec, n_sids, procs = oracle_sample(cfg, users)
+        line["cpu_baseline"] = {"value": n_sids / sec, "unit": UNIT, "cores": procs, "kind": "oracle",
+                                "sample": f"users {users} of {cfg.B} of {cfg.name} (prefix lengths "
+                                          f"{[int(lens[u]) for u in users]}: the shortest ones -- the oracle replicates "
+                                          f"every beam's whole KV cache), all {cfg.d} decode steps, one process per user, "
+                                          f"{sec:.1f} s wall",
+                                "cpu": cpu_info()}
+    # ---- the other configurations (same protocol, rank 0, N = 1) --------------------------------
+    names = [n for n in args.per_config.split(",") if n and n != cfg.name]
+    if world == 1 and names:
+        del hosts, passes, calls, call_all, bufs, h0
+        torch.cuda.empty_cache()
+        per = {}
+        for n in names:
+            try:
+                per[n] = measure_config(torch, wl.get_config(n), dev, pk, args)
+            except Exception as e:  # noqa: BLE001  (one config failing must not lose the headline)
+                per[n] = {"error": repr(e)}
+        line["per_config"] = per
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()
@@ -592,6 +826,8 @@ def main():
     args = parse_args()
     if args.calibrate:
         return run_calibrate()
+    if args.traffic_from:
+        return run_traffic_from(args)
     if args.workload == "cfg3_decoder":
         return run_cfg3_decoder(args)
     cfg = wl.get_config(args.workload)

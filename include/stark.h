@@ -244,8 +244,17 @@ int stark_decode_step(const stark_shape_t* shape, const void* q, int n_q, int le
  * Caller passes W_out = min(W, W_in*C); widths may differ per level
  * (512, 512, 1024).
  * ws, ws_bytes   workspace of stark_workspace_bytes(STARK_CALL_BEAM_TOPK, ...)
+ *                bytes (0 for small candidate sets: ws may then be NULL).  Large
+ *                candidate sets are spread over all SMs of the GPU; the CTAs of a
+ *                user meet through counters and lists in the workspace.  THE
+ *                WORKSPACE MUST BE ZERO-FILLED BEFORE ITS FIRST USE (one
+ *                cudaMemset after allocation); every call leaves it zero-filled
+ *                again, so it can be reused by any later call that is ordered
+ *                after this one (same stream / same graph); calls that may run
+ *                concurrently need a workspace each.
  * Errors: INVALID_ARG (null pointers, non-positive dims, W_out > W_in*C,
- * W_out > 4096, W_in*C >= 2^31), WORKSPACE, CUDA.
+ * W_out > 4096 -- reading R7: PAPER.md:306 needs at most 1024 --, W_in*C >= 2^31),
+ * WORKSPACE (ws NULL or smaller than stark_workspace_bytes says), CUDA.
  */
 int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_in, int C,
                     int W_out, float* out_score, int32_t* out_parent, int32_t* out_code,
@@ -271,7 +280,9 @@ int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_
  * stark_beam_topk_logits runs both (one launch when W_in == 1 and C <= 512, i.e.
  * decode step 0: the one-CTA selection kernel normalises its single row itself;
  * two launches otherwise); ws, ws_bytes = workspace of
- * stark_workspace_bytes(shape (B only), STARK_CALL_BEAM_TOPK_LOGITS, W_in, C).
+ * stark_workspace_bytes(shape (B only), STARK_CALL_BEAM_TOPK_LOGITS, W_in, C),
+ * zero-filled before its first use like stark_beam_topk's (left zero-filled
+ * except for the per-beam offsets at its front, which every call rewrites).
  * Errors: as stark_beam_topk; the workspace is always required.
  */
 int stark_logits_row_offset(const float* logits, const float* score_or_null, int64_t rows, int C,
@@ -308,9 +319,11 @@ int stark_kv_append_reorg(const stark_shape_t* shape, int level, int n_new,
 /* ---------------------------------------------------------------------------
  * Sizes the caller must allocate (host arithmetic only).
  */
-/* Workspace bytes for `call`.  For STARK_CALL_BEAM_TOPK pass n_q = W_in,
- * total_tokens = C and shape->B = B (other shape fields ignored); the other
- * calls currently need none and return 0.  Returns 0 on invalid input. */
+/* Workspace bytes for `call`.  For STARK_CALL_BEAM_TOPK and
+ * STARK_CALL_BEAM_TOPK_LOGITS pass n_q = W_in, total_tokens = C and
+ * shape->B = B (other shape fields ignored; the size does not depend on
+ * W_out); the other calls currently need none and return 0.  Returns 0 on
+ * invalid input.  See stark_beam_topk for the zero-fill rule. */
 size_t stark_workspace_bytes(const stark_shape_t* shape, int call, int n_q, int total_tokens);
 /* Bytes of ONE of k_suffix / v_suffix: d*B*Wmax*Hkv*D*elem. */
 size_t stark_suffix_bytes(const stark_shape_t* shape);

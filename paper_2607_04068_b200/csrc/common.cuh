@@ -121,6 +121,11 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
 // R22); only where topk_can_fold_lse() says so (one row per user, small enough for the one-CTA kernel).
 bool topk_can_fold_lse(int W_in, int C);
 size_t topk_workspace_bytes(int B, int W_in, int C);
+// topk_grid.cu: large candidate sets on the whole GPU; STARK_ERR_UNSUPPORTED = not served, use launch_topk's kernels
+size_t topk_grid_workspace_bytes(int B, int W_in, int C);
+int launch_topk_grid(const float* logp, const float* score, int B, int W_in, int C, int W_out,
+                     float* out_score, int32_t* out_parent, int32_t* out_code, void* ws, size_t ws_bytes,
+                     cudaStream_t st);
 int launch_row_offset(const float* logits, const float* score, long long rows, int C, float* offset,
                       cudaStream_t st);
 

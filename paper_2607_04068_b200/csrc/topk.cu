@@ -994,12 +994,12 @@ int next_pow2(int x) { int p = 1; while (p < x) p <<= 1; return p; }
 
 }  // namespace
 
-size_t topk_workspace_bytes(int, int, int) { return 0; }
+size_t topk_workspace_bytes(int B, int W_in, int C) { return topk_grid_workspace_bytes(B, W_in, C); }
 
 bool topk_can_fold_lse(int W_in, int C) { return W_in == 1 && C <= kSmallMax; }
 
 int launch_topk(const float* logp, const float* score, int B, int W_in, int C, int W_out,
-                float* out_score, int32_t* out_parent, int32_t* out_code, void*, size_t,
+                float* out_score, int32_t* out_parent, int32_t* out_code, void* ws, size_t ws_bytes,
                 cudaStream_t st, bool fold_lse) {
     const long long N = (long long)W_in * C;
     if (fold_lse && !topk_can_fold_lse(W_in, C)) return STARK_ERR_INVALID_ARG;
@@ -1032,6 +1032,11 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
                                                                                  out_score, out_parent, out_code);
         STARK_LAUNCH_CHECK();
         return STARK_OK;
+    }
+    // large candidate sets: the whole GPU on every user (topk_grid.cu); UNSUPPORTED = shape not served there
+    if (ws) {
+        const int rc = launch_topk_grid(logp, score, B, W_in, C, W_out, out_score, out_parent, out_code, ws, ws_bytes, st);
+        if (rc != STARK_ERR_UNSUPPORTED) return rc;
     }
     const int cap = next_pow2(W_out) * 2 < 128 ? 128 : next_pow2(W_out) * 2;  // sort buffer entries
     // pruning pays once a thread holds many keys (>= 16: slices of 8192) and needs K <= the 2048 buckets of a CTA

@@ -92,15 +92,35 @@ class StarkLayer:
         return self._partials(n_q)[0]
 
 
+_WS_CACHE = {}
+
+
+def topk_workspace(B: int, W_in: int, C: int, device, logits: bool = False) -> Optional[torch.Tensor]:
+    """Workspace of stark_beam_topk (logits: stark_beam_topk_logits) for this shape, sized by the library's own
+    helper.  include/stark.h: it must be ZERO before its first use and every call leaves it zero, so one cached
+    buffer per (device, size) serves all calls that are ordered on one stream."""
+    shape = sb.make_shape(B=B, Hq=1, Hkv=1, D=64, d=1, Wmax=W_in, dtype=torch.float32)
+    n = sb.stark_workspace_bytes(shape, sb.CALL_BEAM_TOPK_LOGITS if logits else sb.CALL_BEAM_TOPK, W_in, C)
+    if n == 0:
+        return None
+    key = (str(device), n, logits)
+    if key not in _WS_CACHE:
+        _WS_CACHE[key] = torch.zeros(n, dtype=torch.uint8, device=device)
+    return _WS_CACHE[key]
+
+
 def beam_topk(logp: torch.Tensor, score: Optional[torch.Tensor], W_out: int,
-              out: Optional[Tuple[torch.Tensor, torch.Tensor, torch.Tensor]] = None):
+              out: Optional[Tuple[torch.Tensor, torch.Tensor, torch.Tensor]] = None,
+              ws: Optional[torch.Tensor] = None):
     """logp[B,W_in,C] fp32, score[B,W_in] fp32 or None -> (score, parent, code) [B,W_out]."""
     B, W_in, C = logp.shape
     if out is None:
         out = (torch.empty((B, W_out), dtype=torch.float32, device=logp.device),
                torch.empty((B, W_out), dtype=torch.int32, device=logp.device),
                torch.empty((B, W_out), dtype=torch.int32, device=logp.device))
-    sb.stark_beam_topk(logp, score, B, W_in, C, W_out, out[0], out[1], out[2])
+    if ws is None:
+        ws = topk_workspace(B, W_in, C, logp.device)
+    sb.stark_beam_topk(logp, score, B, W_in, C, W_out, out[0], out[1], out[2], ws)
     return out
 
 
@@ -115,8 +135,6 @@ def beam_topk_logits(logits: torch.Tensor, score: Optional[torch.Tensor], W_out:
                torch.empty((B, W_out), dtype=torch.int32, device=logits.device),
                torch.empty((B, W_out), dtype=torch.int32, device=logits.device))
     if ws is None:
-        shape = sb.make_shape(B=B, Hq=1, Hkv=1, D=64, d=1, Wmax=W_in, dtype=torch.float32)
-        ws = torch.empty(sb.stark_workspace_bytes(shape, sb.CALL_BEAM_TOPK_LOGITS, W_in, C), dtype=torch.uint8,
-                         device=logits.device)
+        ws = topk_workspace(B, W_in, C, logits.device, logits=True)
     sb.stark_beam_topk_logits(logits, score, B, W_in, C, W_out, out[0], out[1], out[2], ws)
     return out

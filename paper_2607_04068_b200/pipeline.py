@@ -34,11 +34,11 @@ class DecodePass:
         # from_logits: `logp` holds RAW per-level logits and the selection is stark_beam_topk_logits (A3':
         # the log-softmax normaliser is folded into the beam score, two launches per level)
         self.from_logits = from_logits
-        self.topk_ws = None
-        if from_logits:
-            shp = sb.make_shape(B, 1, 1, 64, 1, max(self.n_q), torch.float32)
-            need = max(sb.stark_workspace_bytes(shp, sb.CALL_BEAM_TOPK_LOGITS, self.n_q[t], C) for t in range(d))
-            self.topk_ws = torch.empty(need, dtype=torch.uint8, device=dev)
+        # one workspace for every level's selection (zero before its first use, left zero by every call)
+        shp = sb.make_shape(B, 1, 1, 64, 1, max(self.n_q), torch.float32)
+        call = sb.CALL_BEAM_TOPK_LOGITS if from_logits else sb.CALL_BEAM_TOPK
+        need = max(sb.stark_workspace_bytes(shp, call, self.n_q[t], C) for t in range(d))
+        self.topk_ws = torch.zeros(need, dtype=torch.uint8, device=dev) if need else None
         self.out = [torch.empty_like(q[t]) for t in range(d)]
         self.sel = [(torch.empty((B, w), dtype=torch.float32, device=dev),
                      torch.empty((B, w), dtype=torch.int32, device=dev),
@@ -66,7 +66,7 @@ class DecodePass:
     def select(self, t: int, score: Optional[torch.Tensor]):
         if self.from_logits:
             return beam_topk_logits(self.logp[t], score, self.widths[t], out=self.sel[t], ws=self.topk_ws)
-        return beam_topk(self.logp[t], score, self.widths[t], out=self.sel[t])
+        return beam_topk(self.logp[t], score, self.widths[t], out=self.sel[t], ws=self.topk_ws)
 
     def result(self) -> Dict[str, List[torch.Tensor]]:
         return {"score": [s[0] for s in self.sel], "parent": [s[1] for s in self.sel],

@@ -97,3 +97,15 @@ def test_no_cpu_fallback(L):
     p = ctypes.c_void_p(16)
     rc = L.stark_beam_topk(p, None, 1, 2, 4, 2, p, p, p, None, 0, None)
     assert rc in (-2, -4)
+
+
+def test_topk_workspace_rule(L):
+    """Large candidate sets need the (zero-filled) workspace stark_workspace_bytes reports; small ones need none."""
+    p = ctypes.c_void_p(16)
+    sh = sb.make_shape(2, 1, 1, 64, 1, 512, torch.float32)
+    assert sb.stark_workspace_bytes(sh, sb.CALL_BEAM_TOPK, 1, 256) == 0
+    need = sb.stark_workspace_bytes(sh, sb.CALL_BEAM_TOPK, 512, 8192)
+    assert need > 0 and need == sb.stark_workspace_bytes(sh, sb.CALL_BEAM_TOPK, 512, 8192)
+    assert L.stark_beam_topk(p, None, 2, 512, 8192, 512, p, p, p, None, 0, None) == -3        # no workspace
+    assert L.stark_beam_topk(p, None, 2, 512, 8192, 512, p, p, p, p, need - 1, None) == -3    # too small
+    assert sb.stark_workspace_bytes(sh, sb.CALL_BEAM_TOPK_LOGITS, 512, 8192) > need           # + the per-beam offsets
