@@ -22,15 +22,16 @@
 //      filtered the same way.  Unsorted parents make L loose: when the list fills up, the CTA re-tightens its
 //      own bound from the list (its K-th largest entry is again a valid bound) and compacts -- a streaming top-K.
 //   4. Every CTA writes its survivors, as composites (~ord(key) . index), and their count to its own segment of
-//      the user's list in the workspace; the LAST CTA of the user to finish (a counter) ranks the composites of
-//      all segments -- all distinct, so the order "key descending, index ascending" is their plain ascending
-//      order and the result does not depend on arrival order -- and the entries of rank < K write their
-//      (score, parent, code) row.  Ranking = bucketing on the top 11 bits of the composites' range (a counting
-//      sort) + counting inside each bucket: no sorting network.  More than 4096 survivors are first cut down by
-//      exact radix passes; massive exact ties inside one bucket fall back to a register/merge sort; a CTA that
-//      lost survivors (list overflow: K keys of -inf, all keys equal, ...) makes the last CTA run the same exact
-//      selection over ALL keys of the user, read again by that one CTA: slow, never wrong.
-//   5. The last CTA zeroes the user's workspace state, so the workspace only has to be zero ONCE, before its
+//      the user's list in the workspace and arrives at the user's second barrier.  Then EVERY CTA copies the
+//      whole list (1-2 K composites) into shared memory and ranks its OWN survivors against it, a warp per
+//      survivor: the composites are all distinct, so the order "key descending, index ascending" is their plain
+//      ascending order, rank = number of smaller composites, and the survivors of rank < K write their (score,
+//      parent, code) row directly -- no sort, no serial tail, a result independent of arrival order.
+//      Exceptional cases are finished by the last CTA to arrive alone: more than 8192 survivors (cut down by
+//      exact radix passes, then ranked by bucketing), or a CTA that lost survivors (list overflow: K keys of
+//      -inf, all keys equal, ...): the same exact selection over ALL keys of the user, read again by that one
+//      CTA: slow, never wrong.
+//   5. The last CTA to finish zeroes the user's workspace state, so the workspace only has to be zero ONCE, before its
 //      first use (include/stark.h).
 // Algorithmic HBM bytes: 4 per candidate (read once) + 4 per input beam + 12 per selected beam.
 #include "common.cuh"
@@ -48,12 +49,13 @@ constexpr int kBins = 2048;                       // 11-bit digits
 constexpr int kCoarse = 64;
 constexpr int kSvCap = 4096;                      // survivor list entries per CTA
 constexpr int kEmitMax = 2048;                    // a CTA emits at most this many survivors
-constexpr int kSortCap = 4096;                    // composites the last CTA ranks in shared memory
+constexpr int kSortCap = 4096;                    // composites the last CTA ranks in shared memory (exceptional path)
+constexpr int kRankCap = 8192;                    // survivors of a user every CTA ranks against (fills the key cache)
 constexpr int kBucketMax = 192;                   // largest bucket ranked by counting (beyond: massive ties, sort)
 constexpr int kMaxK = 1024;                       // W_out served by this path (kSvCap / 2 >= K for the re-tightening)
 constexpr int kPubPerThread = 16;                 // published maxima a thread reads
 constexpr int kMaxGroups = kPubPerThread * kThreads;   // published maxima per user at most (8192)
-constexpr uint32_t kLost = 0xffffffffu;           // segment count of a CTA that lost survivors
+constexpr uint32_t kOverflow = 0x00400000u;       // added to a user's count by a CTA that lost survivors (> any real count; 512 of them do not wrap)
 constexpr long long kGridMinN = 131072;           // candidates per user from which this path is tried (measured)
 constexpr int kGridMaxCtas = 512;                 // CTAs of one launch at most (workspace sizing; 2 x 148 on B200)
 
@@ -73,11 +75,22 @@ __device__ unsigned long long g_topk_prof[1024 * 16];
 #define PROF_VAL(i, v) do {} while (0)
 #endif
 
-struct UserState {                                // zero before the launch, zero after it
-    unsigned long long release;                   // (1 << 32) | bound, written once by the last CTA to arrive
-    uint32_t arrived, done, pad[4];
+// Per-user counters, each on a cache line of its own (zero before the launch, zero after it).  The release words
+// are NOT here: hundreds of CTAs polling one address saturate that L2 slice and delay the very atomics they wait
+// for (measured: 5 us per barrier), so every CTA polls a slot of its own (RelSlot), which the releasing CTA writes.
+struct UserState {
+    uint32_t arrived_a, pad0[31];
+    uint32_t arrived_b, pad1[31];
+    uint32_t done, pad2[31];
+    uint32_t count, pad3[31];                     // survivors appended to the user's list (+ kOverflow if any were lost)
 };
-static_assert(sizeof(UserState) == 32, "workspace layout");
+static_assert(sizeof(UserState) == 512, "workspace layout");
+struct RelSlot {                                  // one per CTA, 64 bytes apart
+    unsigned long long a;                         // (1 << 32) | bound: written by the user's last CTA at barrier A
+    unsigned long long b;                         // (1 << 63) | mode << 32 | survivors: ... at barrier B
+    unsigned long long pad[6];
+};
+static_assert(sizeof(RelSlot) == 64, "workspace layout");
 
 struct Shared {
     uint32_t hist[kBins];
@@ -93,7 +106,8 @@ struct Shared {
 constexpr size_t kSharedBytes = ((sizeof(Shared) + 15) / 16) * 16;
 constexpr size_t kSmemBytes = kSharedBytes + (size_t)kBatch * 4 + (size_t)kSvCap * 8;
 static_assert((size_t)kBatch * 4 >= (size_t)kSortCap * 16, "the key cache holds the last CTA's two composite arrays");
-static_assert((size_t)kSvCap * 8 >= (size_t)(kBins + 1 + kGridMaxCtas + 1 + kThreads) * 4, "bucket bases + segment offsets + scan");
+static_assert((size_t)kBatch * 4 >= (size_t)kRankCap * 8, "the key cache holds the user's whole survivor list");
+static_assert((size_t)kSvCap * 8 >= (size_t)(kBins + 1 + kThreads) * 4, "bucket bases + scan words");
 
 __device__ __forceinline__ uint32_t ord_of(float key) {
     uint32_t b = __float_as_uint(key);
@@ -108,6 +122,17 @@ __device__ __forceinline__ unsigned long long ld_acquire(const unsigned long lon
     unsigned long long v;
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
+}
+__device__ __forceinline__ uint32_t ld_acquire32(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+// arrive at a counter: release this CTA's writes (ordered before by the CTA barrier), acquire the others'
+__device__ __forceinline__ uint32_t atom_add_acq_rel(uint32_t* p, uint32_t v) {
+    uint32_t old;
+    asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], %2;" : "=r"(old) : "l"(p), "r"(v) : "memory");
+    return old;
 }
 __device__ __forceinline__ void st_release(unsigned long long* p, unsigned long long v) {
     asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
@@ -176,53 +201,43 @@ __device__ __forceinline__ void coarse_from_hist(Shared& sh) {
     if ((lane & 7) == 0) sh.coarse[tid >> 3] = c4;
 }
 
-// K-th largest of the NON-ZERO values v[0], v[stride], ..., v[(n-1)*stride] (shared memory; 0 = absent), resolved
-// to 22 bits of their range: a value L such that at least K of them are >= L (and, unless the range exceeds 2^22,
-// exactly the K-th largest).  0 if there are fewer than K non-zero values.  Block-uniform result.
-__device__ __noinline__ uint32_t kth_largest(Shared& sh, const uint32_t* v, int n, int stride, uint32_t K) {
+// A value L such that at least K of the NON-ZERO values among the block's kNV * kThreads register-held values `v`
+// (0 = absent) are >= L, within 2^-11 of their range of the K-th largest; 0 if there are fewer than K non-zero
+// values.  Bisection on the value, counting by warp votes: shared-memory atomics cost ~2 cycles per VALUE on this
+// machine (a 2048-bin histogram of 4.7 K values took 3 us), a bisection step ~0.06 us.  Block-uniform result.
+template <int kNV>
+__device__ __forceinline__ uint32_t kth_largest(Shared& sh, const uint32_t (&v)[kNV], uint32_t K) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     uint32_t vmax = 0u, vmin = 0xffffffffu, cnt = 0u;
-#pragma unroll 4
-    for (int i = tid; i < n; i += kThreads) {
-        const uint32_t x = v[i * stride];
-        if (x) { vmax = max(vmax, x); vmin = min(vmin, x); ++cnt; }
-    }
+#pragma unroll
+    for (int x = 0; x < kNV; ++x)
+        if (v[x]) { vmax = max(vmax, v[x]); vmin = min(vmin, v[x]); ++cnt; }
     vmax = __reduce_max_sync(0xffffffffu, vmax);
     vmin = __reduce_min_sync(0xffffffffu, vmin);
     cnt = __reduce_add_sync(0xffffffffu, cnt);
     if (lane == 0) { sh.wmax[warp] = vmax; sh.wmin[warp] = vmin; sh.wcnt[warp] = cnt; }
-    zero_hist(sh);
     __syncthreads();
     vmax = __reduce_max_sync(0xffffffffu, lane < kWarps ? sh.wmax[lane] : 0u);
     vmin = __reduce_min_sync(0xffffffffu, lane < kWarps ? sh.wmin[lane] : 0xffffffffu);
     cnt = __reduce_add_sync(0xffffffffu, lane < kWarps ? sh.wcnt[lane] : 0u);
-    if (cnt < K) { __syncthreads(); return 0u; }
-    const uint32_t span = vmax - vmin;
-    const int nb = span ? 32 - __clz((int)span) : 0;
-    uint32_t edge = vmin, rem = K, bin = 0;
-    int shl = nb;                                 // unresolved low bits of (v - vmin)
+    __syncthreads();
+    if (cnt < K) return 0u;
+    // invariant: count(v >= lo) >= K, count(v >= hi) < K  (hi = vmax + 1 conceptually: count 0 < K)
+    uint32_t lo = vmin, hi = vmax;                // hi is tested with ">" below so that vmax itself stays eligible
+    uint32_t n_lo = cnt;
 #pragma unroll 1
-    for (int level = 0; level < 2 && shl > 0; ++level) {
-        const int w = min(11, shl), shl2 = shl - w;
-        const uint32_t mask = (1u << w) - 1u;
-        if (level) { zero_hist(sh); __syncthreads(); }
-#pragma unroll 4
-        for (int i = tid; i < n; i += kThreads) {
-            const uint32_t x = v[i * stride];
-            if (x && (level == 0 || ((x - vmin) >> shl) == bin)) atomicAdd(&sh.hist[((x - vmin) >> shl2) & mask], 1u);
-        }
+    for (int it = 0; it < 11 && hi - lo > 1u && n_lo > K + (K >> 5); ++it) {
+        const uint32_t mid = lo + ((hi - lo) >> 1);
+        uint32_t c = 0;
+#pragma unroll
+        for (int x = 0; x < kNV; ++x) c += __popc(__ballot_sync(0xffffffffu, v[x] >= mid));   // (0 < mid always)
+        if (lane == 0) sh.hist[(it & 1) * kWarps + warp] = c;
         __syncthreads();
-        coarse_from_hist(sh);
-        __syncthreads();
-        if (warp == 0) block_select(sh, rem);
-        __syncthreads();
-        bin = (level ? (bin << w) : 0u) | sh.sel_bin;
-        rem = sh.sel_rem;
-        shl = shl2;
-        edge = vmin + (bin << shl);
-        __syncthreads();                          // (sel_bin / hist are reused)
+        c = __reduce_add_sync(0xffffffffu, lane < kWarps ? sh.hist[(it & 1) * kWarps + lane] : 0u);
+        if (c >= K) { lo = mid; n_lo = c; } else hi = mid;
     }
-    return edge;
+    __syncthreads();
+    return lo;
 }
 
 // block-wide (max, min) of one 64-bit value per thread; ends with a barrier
@@ -485,17 +500,19 @@ __device__ __noinline__ void append4(Shared& sh, uint2* sv, float thr, float4 k,
 // raise `bound` and compact the list.  Returns the new length.
 __device__ __noinline__ uint32_t retighten(Shared& sh, uint2* sv, uint32_t cnt, uint32_t& bound, uint32_t K) {
     const int tid = threadIdx.x;
-    bound = max(bound, kth_largest(sh, reinterpret_cast<const uint32_t*>(sv), (int)cnt, 2, K));
     uint2 mine[kSvCap / kThreads];
+    uint32_t ov[kSvCap / kThreads];
 #pragma unroll
     for (int x = 0; x < kSvCap / kThreads; ++x) {
         const uint32_t e = tid + x * kThreads;
         mine[x] = e < cnt ? sv[e] : make_uint2(0u, 0u);       // (ord of a real key is never 0)
+        ov[x] = mine[x].x;
     }
+    bound = max(bound, kth_largest<kSvCap / kThreads>(sh, ov, K));
     __syncthreads();
 #pragma unroll
     for (int x = 0; x < kSvCap / kThreads; ++x)
-        if (mine[x].x && mine[x].x >= bound) sv[atomicAdd(&sh.sv_count2, 1u)] = mine[x];
+        if (ov[x] && ov[x] >= bound) sv[atomicAdd(&sh.sv_count2, 1u)] = mine[x];
     __syncthreads();
     const uint32_t c2 = sh.sv_count2;
     __syncthreads();
@@ -506,51 +523,22 @@ __device__ __noinline__ uint32_t retighten(Shared& sh, uint2* sv, uint32_t cnt, 
 
 // The user's last CTA: rank the survivors of all S segments, write the result, leave the workspace zeroed.
 __device__ __noinline__ void finish_user(Shared& sh, unsigned long long* ent, uint32_t* words, const Keys& ks,
-                                         const Out& out, uint32_t K, int S, int G, UserState* st, uint32_t* upub,
-                                         uint32_t* ucnt, const unsigned long long* ulist) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+                                         const Out& out, uint32_t K, uint32_t n_list, bool lost, int S, int G,
+                                         UserState* st, uint32_t* upub, const unsigned long long* ulist, RelSlot* urel) {
+    const int tid = threadIdx.x;
     unsigned long long* bucketed = ent + kSortCap;                            // kSortCap composites
     uint32_t* base = words;                                                   // kBins + 1 bucket bases
-    uint32_t* seg_off = base + kBins + 1;                                     // S + 1 segment offsets
-    uint32_t* part = seg_off + kGridMaxCtas + 1;                              // kThreads scan words
-    // segment offsets: exclusive prefix over the S counts (S <= kThreads)
-    uint32_t n_list;
-    {
-        const uint32_t mine = tid < S ? __ldcg(ucnt + tid) : 0u;
-        const bool any_lost = __syncthreads_or(mine == kLost);
-        uint32_t inc = mine;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
-        }
-        if (lane == 31) sh.wcnt[warp] = inc;
-        __syncthreads();
-        uint32_t before = 0;
-#pragma unroll 1
-        for (int w = 0; w < warp; ++w) before += sh.wcnt[w];
-        if (tid < S) seg_off[tid] = before + inc - mine;
-        if (tid == S - 1) seg_off[S] = before + inc;
-        __syncthreads();
-        n_list = any_lost ? kLost : seg_off[S];
-    }
-    // flat entry i of the list: binary search of its segment
-    auto list_entry = [&](uint32_t i) -> unsigned long long {
-        int lo = 0, hi = S;                                   // seg_off[lo] <= i < seg_off[hi]
-#pragma unroll 1
-        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (seg_off[mid] <= i) lo = mid; else hi = mid; }
-        return __ldcg(ulist + (size_t)lo * kEmitMax + (i - seg_off[lo]));
-    };
+    uint32_t* part = base + kBins + 1;                                        // kThreads scan words
     int n_g;
-    if (n_list != kLost && n_list >= K && n_list <= (uint32_t)kSortCap) {
+    if (!lost && n_list >= K && n_list <= (uint32_t)kSortCap) {
 #pragma unroll 4
-        for (uint32_t i = tid; i < n_list; i += kThreads) ent[i] = list_entry(i);
+        for (uint32_t i = tid; i < n_list; i += kThreads) ent[i] = __ldcg(ulist + i);
         n_g = (int)n_list;
         __syncthreads();
-    } else if (n_list != kLost && n_list >= K) {
+    } else if (!lost && n_list >= K) {
         n_g = select_gather(sh, ent, [&](auto&& put) {
-#pragma unroll 2
-            for (uint32_t i = tid; i < n_list; i += kThreads) put(list_entry(i));
+#pragma unroll 4
+            for (uint32_t i = tid; i < n_list; i += kThreads) put(__ldcg(ulist + i));
         }, n_list, K);
     } else {
         // a CTA lost survivors: the same exact selection over ALL keys of the user, read again by this CTA
@@ -574,22 +562,18 @@ __device__ __noinline__ void finish_user(Shared& sh, unsigned long long* ent, ui
             n_g = (int)ks.N;
         }
     }
-    PROF(7);
-    PROF_VAL(9, n_list);
     rank_emit(sh, ent, bucketed, base, part, n_g, K, ks, out);
-    PROF(14);
     // leave the workspace zeroed
     for (int i = tid; i < S * G; i += kThreads) upub[i] = 0u;
-    if (tid < S) ucnt[tid] = 0u;
+    if (tid < S) { urel[tid].a = 0ull; urel[tid].b = 0ull; }
     if (tid < (int)(sizeof(UserState) / 4)) reinterpret_cast<uint32_t*>(st)[tid] = 0u;
-    PROF(8);
 }
 
 __global__ void __launch_bounds__(kThreads, 2)
 topk_grid_kernel(const float* __restrict__ logp, const float* __restrict__ score, int W_in, int C, int c_shift,
                  int W_out, float* __restrict__ out_score, int32_t* __restrict__ out_parent,
                  int32_t* __restrict__ out_code, int S, int G, UserState* __restrict__ state,
-                 uint32_t* __restrict__ pub, uint32_t* __restrict__ seg_cnt, unsigned long long* __restrict__ list) {
+                 uint32_t* __restrict__ pub, unsigned long long* __restrict__ list, RelSlot* __restrict__ rel) {
     const int s = blockIdx.x, u = blockIdx.y;
     const int tid = threadIdx.x;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -605,8 +589,8 @@ topk_grid_kernel(const float* __restrict__ logp, const float* __restrict__ score
     const uint32_t N = ks.N, K = (uint32_t)W_out;
     UserState* st = state + u;
     uint32_t* upub = pub + (size_t)u * kMaxGroups;
-    uint32_t* ucnt = seg_cnt + (size_t)u * S;                  // survivors per CTA of this user
-    unsigned long long* ulist = list + (size_t)u * S * kEmitMax;   // segment s at s * kEmitMax
+    unsigned long long* ulist = list + (size_t)u * S * kEmitMax;   // the user's survivor list (S * kEmitMax entries)
+    RelSlot* urel = rel + (size_t)u * S;                       // release slot of CTA s at urel[s]
     const int n_chunks = (int)((N + kChunk - 1) / kChunk);
     const int my_chunks = s < n_chunks ? (n_chunks - s + S - 1) / S : 0;
     const float ninf = __int_as_float(0xff800000);
@@ -652,24 +636,29 @@ topk_grid_kernel(const float* __restrict__ logp, const float* __restrict__ score
         if ((tid & (gsz - 1)) == 0) __stcg(upub + (size_t)s * G + tid / gsz, gmax);
     }
     if (kUnroll < my_chunks) load_batch(kUnroll);         // the next batch is in flight across the barrier
-    __threadfence();
+    // barrier pattern: the CTA barrier orders every thread's writes before thread 0's fence + atomic
     __syncthreads();
-    if (tid == 0) sh.flag = atomicAdd(&st->arrived, 1u) == (uint32_t)(S - 1) ? 1u : 0u;
+    if (tid == 0) sh.flag = atom_add_acq_rel(&st->arrived_a, 1u) == (uint32_t)(S - 1) ? 1u : 0u;
     __syncthreads();
     uint32_t bound;
+    PROF(2);
     if (sh.flag) {                                        // everyone's maxima are published
-        __threadfence();
-        const int M = S * G;                              // <= kMaxGroups: fits the (still empty) survivor list
-        uint32_t* stage = reinterpret_cast<uint32_t*>(sv);
-#pragma unroll 4
-        for (int i = tid; i < M; i += kThreads) stage[i] = __ldcg(upub + i);
+        const int M = S * G;                              // <= kMaxGroups = kPubPerThread * kThreads
+        uint32_t pv[kPubPerThread];
+#pragma unroll
+        for (int x = 0; x < kPubPerThread; ++x) {         // all loads in flight at once
+            const int i = tid + x * kThreads;
+            pv[x] = i < M ? __ldcg(upub + i) : 0u;
+        }
+        PROF(11);
+        bound = kth_largest<kPubPerThread>(sh, pv, K);
+        PROF(12);
         __syncthreads();
-        bound = kth_largest(sh, stage, M, 1, K);
-        if (tid == 0) st_release(&st->release, (1ull << 32) | bound);
+        if (tid < S) st_release(&urel[tid].a, (1ull << 32) | bound);
     } else {
         if (tid == 0) {
             unsigned long long r;
-            do { r = ld_acquire(&st->release); } while (r == 0ull);
+            while ((r = ld_acquire(&urel[s].a)) == 0ull) __nanosleep(20);
             sh.bound = (uint32_t)r;
         }
         __syncthreads();
@@ -698,11 +687,11 @@ topk_grid_kernel(const float* __restrict__ logp, const float* __restrict__ score
         if (++since_check < 4 && k0 + kUnroll < my_chunks) continue;
         since_check = 0;
         __syncthreads();
-        const uint32_t cnt = sh.sv_count;                // (block-uniform)
+        const uint32_t c1 = sh.sv_count;                 // (block-uniform)
         __syncthreads();
-        if (cnt > (uint32_t)kSvCap) { lost = true; break; }
-        if (cnt > (uint32_t)(kSvCap / 2)) {
-            if (retighten(sh, sv, cnt, bound, K) > (uint32_t)(kSvCap / 2)) { lost = true; break; }
+        if (c1 > (uint32_t)kSvCap) { lost = true; break; }
+        if (c1 > (uint32_t)(kSvCap / 2)) {
+            if (retighten(sh, sv, c1, bound, K) > (uint32_t)(kSvCap / 2)) { lost = true; break; }
             thr = bound <= 0x007fffffu ? ninf : ord_inv(bound);
         }
     }
@@ -724,23 +713,87 @@ topk_grid_kernel(const float* __restrict__ logp, const float* __restrict__ score
         if (cnt > (uint32_t)kSvCap) lost = true;
         else if (cnt > (uint32_t)kEmitMax) { cnt = retighten(sh, sv, cnt, bound, K); if (cnt > (uint32_t)kEmitMax) lost = true; }
     }
-    // ---- 4. the CTA's segment of the user's list + its count; the last CTA to finish takes over -----------
-    if (!lost)
-        for (uint32_t e = tid; e < cnt; e += kThreads)
-            __stcg(ulist + (size_t)s * kEmitMax + e, ((unsigned long long)(~sv[e].x) << 32) | sv[e].y);
-    if (tid == 0) __stcg(ucnt + s, lost ? kLost : cnt);
+    // ---- 4. append to the user's list (one reservation per CTA); second barrier ------------------------------
+    if (tid == 0) sh.cursor = atomicAdd(&st->count, lost ? kOverflow : cnt);
+    __syncthreads();
+    {
+        const uint32_t at = sh.cursor;
+        if (!lost && at + cnt <= (uint32_t)(S * kEmitMax))
+            for (uint32_t e = tid; e < cnt; e += kThreads)
+                __stcg(ulist + at + e, ((unsigned long long)(~sv[e].x) << 32) | sv[e].y);
+    }
     PROF(5);
-    __threadfence();
+    __syncthreads();
+    if (tid == 0) sh.flag = atom_add_acq_rel(&st->arrived_b, 1u) == (uint32_t)(S - 1) ? 1u : 0u;
+    __syncthreads();
+    const bool last_b = sh.flag != 0u;
+    // the last CTA to arrive sees the final count and decides how the user is finished:
+    // mode 0: every CTA ranks a slice of the list; 1: the last CTA alone (too many survivors, or some were lost)
+    uint32_t n_list, mode;
+    if (last_b) {
+        if (tid == 0) sh.sel_rem = __ldcg(&st->count);
+        __syncthreads();
+        n_list = sh.sel_rem;
+        mode = (n_list > (uint32_t)kRankCap || n_list < K) ? 1u : 0u;      // (kOverflow > kRankCap)
+        if (tid < S) st_release(&urel[tid].b, (1ull << 63) | ((unsigned long long)mode << 32) | n_list);
+    } else {
+        if (tid == 0) {
+            unsigned long long r;
+            while ((r = ld_acquire(&urel[s].b)) == 0ull) __nanosleep(20);
+            sh.sel_bin = (uint32_t)(r >> 32) & 1u;
+            sh.sel_rem = (uint32_t)r;
+        }
+        __syncthreads();
+        mode = sh.sel_bin;
+        n_list = sh.sel_rem;
+    }
+    PROF(6);
+    Out out;
+    out.score = out_score; out.parent = out_parent; out.code = out_code; out.row0 = (size_t)u * W_out;
+    if (mode == 1u) {                                    // exceptional: the last CTA finishes the user alone
+        if (!last_b) {
+            if (tid == 0) atomicAdd(&st->done, 1u);      // (this CTA has read its release word)
+            return;
+        }
+        if (tid == 0)
+            while (ld_acquire32(&st->done) < (uint32_t)(S - 1)) __nanosleep(100);   // nobody polls the workspace any more
+        __syncthreads();
+        const bool some_lost = n_list >= kOverflow;
+        finish_user(sh, reinterpret_cast<unsigned long long*>(cache), reinterpret_cast<uint32_t*>(sv), ks, out, K,
+                    n_list, some_lost || n_list > (uint32_t)(S * kEmitMax), S, G, st, upub, ulist, urel);
+        return;
+    }
+    // ---- every CTA: the user's whole list into shared memory, rank a slice of it --------------------------------
+    unsigned long long* ent = reinterpret_cast<unsigned long long*>(cache);   // n_list <= kRankCap composites
+#pragma unroll 4
+    for (uint32_t i = tid; i < n_list; i += kThreads) ent[i] = __ldcg(ulist + i);
+    __syncthreads();
+    PROF(7);
+    PROF_VAL(9, n_list);
+    {   // CTA s ranks the s-th slice of the list (balanced, whatever CTA the survivors came from): a warp per
+        // entry; the composites are distinct, so rank = number of smaller composites
+        const int lane = tid & 31, warp = tid >> 5;
+        const uint32_t per = (n_list + S - 1) / S, e1 = min(n_list, (uint32_t)(s + 1) * per);
+#pragma unroll 1
+        for (uint32_t e = (uint32_t)s * per + warp; e < e1; e += kWarps) {
+            const unsigned long long c = ent[e];
+            uint32_t rk = 0;
+#pragma unroll 4
+            for (uint32_t i = lane; i < n_list; i += 32) rk += ent[i] < c ? 1u : 0u;
+            rk = __reduce_add_sync(0xffffffffu, rk);
+            if (lane == 0 && rk < K) out.put(ks, rk, c);
+        }
+    }
+    PROF(14);
+    // ---- 5. the last CTA to finish leaves the workspace zeroed -----------------------------------------------
     __syncthreads();
     if (tid == 0) sh.flag = atomicAdd(&st->done, 1u) == (uint32_t)(S - 1) ? 1u : 0u;
     __syncthreads();
-    PROF(6);
     if (!sh.flag) return;
-    __threadfence();
-    Out out;
-    out.score = out_score; out.parent = out_parent; out.code = out_code; out.row0 = (size_t)u * W_out;
-    finish_user(sh, reinterpret_cast<unsigned long long*>(cache), reinterpret_cast<uint32_t*>(sv), ks, out, K, S, G, st,
-                upub, ucnt, ulist);
+    for (int i = tid; i < S * G; i += kThreads) upub[i] = 0u;
+    if (tid < S) { urel[tid].a = 0ull; urel[tid].b = 0ull; }
+    if (tid < (int)(sizeof(UserState) / 4)) reinterpret_cast<uint32_t*>(st)[tid] = 0u;
+    PROF(8);
 }
 
 // per device: CTAs of topk_grid_kernel that can be co-resident (a cooperative launch must fit)
@@ -765,9 +818,9 @@ int grid_capacity() {
 
 bool grid_shape_ok(long long N, int C) { return N >= kGridMinN && (C & 3) == 0; }
 
-// workspace: [B] UserState | [B][kMaxGroups] published maxima | [kGridMaxCtas] segment counts |
-//            [kGridMaxCtas][kEmitMax] survivor segments (B * S <= kGridMaxCtas CTAs share them)
-constexpr size_t kWsTail = (size_t)kGridMaxCtas * 4 + (size_t)kGridMaxCtas * kEmitMax * 8;
+// workspace: [B] UserState | [B][kMaxGroups] published maxima | [kGridMaxCtas][kEmitMax] survivor lists |
+//            [kGridMaxCtas] release slots  (the B * S <= kGridMaxCtas CTAs of a launch share the last two)
+constexpr size_t kWsTail = (size_t)kGridMaxCtas * kEmitMax * 8 + (size_t)kGridMaxCtas * sizeof(RelSlot);
 
 }  // namespace
 
@@ -797,8 +850,8 @@ int launch_topk_grid(const float* logp, const float* score, int B, int W_in, int
     char* p = static_cast<char*>(ws);
     UserState* state = reinterpret_cast<UserState*>(p);
     uint32_t* pub = reinterpret_cast<uint32_t*>(p + (size_t)B * sizeof(UserState));
-    uint32_t* seg_cnt = reinterpret_cast<uint32_t*>(p + (size_t)B * (sizeof(UserState) + (size_t)kMaxGroups * 4));
-    unsigned long long* list = reinterpret_cast<unsigned long long*>(seg_cnt + kGridMaxCtas);
+    unsigned long long* list = reinterpret_cast<unsigned long long*>(p + (size_t)B * (sizeof(UserState) + (size_t)kMaxGroups * 4));
+    RelSlot* rel = reinterpret_cast<RelSlot*>(list + (size_t)kGridMaxCtas * kEmitMax);
     int c_shift = -1;
     if ((C & (C - 1)) == 0) { c_shift = 0; while ((1 << c_shift) < C) ++c_shift; }
     cudaLaunchConfig_t cfg = {};
@@ -811,7 +864,7 @@ int launch_topk_grid(const float* logp, const float* score, int B, int W_in, int
     at[0].val.cooperative = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
     STARK_CUDA_TRY(cudaLaunchKernelEx(&cfg, topk_grid_kernel, logp, score, W_in, C, c_shift, W_out, out_score,
-                                      out_parent, out_code, S, G, state, pub, seg_cnt, list));
+                                      out_parent, out_code, S, G, state, pub, list, rel));
     return STARK_OK;
 }
 

@@ -183,3 +183,27 @@ def test_cfg4_full_size_exact_tie_variant():
     logp = (np.round(r.normal(-7, 1.5, (cfg.B, 512, cfg.C)) * 8) / 8).astype(np.float32)
     score = np.sort((np.round(r.normal(-5, 1, (cfg.B, 512)) * 8) / 8).astype(np.float32))[:, ::-1].copy()
     _check(logp, score, 512)
+
+
+def test_grid_path_shapes_and_exceptional_finishes():
+    """Large candidate sets (>= 131072 per user, W_out <= 1024, C % 4 == 0) take the whole-GPU kernel
+    (topk_grid.cu): non-power-of-two codebooks, chunks that span many parent beams, a ragged last chunk, several
+    users; and its exceptional finishes -- every key equal / a sea of -inf (survivor lists overflow: the last CTA
+    re-selects over all keys), unsorted and reversed parent scores (loose bound: more than 8192 survivors, radix
+    passes + bucket ranking by the last CTA), quantised keys (ties inside and across beams)."""
+    r = _rng(10)
+    for (B, W_in, C, W_out) in [(2, 200, 1000, 512), (1, 4096, 64, 256), (3, 100, 1500, 700), (5, 64, 4096, 1024),
+                               (1, 1024, 1024, 1), (2, 512, 512, 1000)]:
+        logits = r.normal(0, 2, (B, W_in, C))
+        logp = (logits - np.log(np.exp(logits).sum(-1, keepdims=True))).astype(np.float32)
+        score = np.sort(r.normal(-8, 2, (B, W_in)).astype(np.float32))[:, ::-1].copy()
+        _check(logp, score, W_out)
+        _check(logp, score[:, ::-1].copy(), W_out)                       # best parent last
+        _check(logp, r.permutation(score.T).T.copy(), W_out)             # unsorted parents
+        _check((np.round(logp * 4) / 4).astype(np.float32), (np.round(score * 4) / 4).astype(np.float32), W_out)
+    _check(np.full((2, 512, 512), -1.0, np.float32), None, 300)          # all equal: index order only
+    z = np.full((2, 256, 1024), -np.inf, np.float32)
+    z[0, 3, 10:20] = -1.5; z[1, :, 7] = -2.0                             # 10 / 256 finite keys, the rest -inf
+    _check(z, np.zeros((2, 256), np.float32), 512)
+    z2 = np.zeros((1, 512, 512), np.float32); z2[0, ::2] = -0.0          # signed zeros, all equal
+    _check(z2, None, 1024)
