@@ -39,3 +39,6 @@ from .beam_search import conventional_beam_search, BeamTrace  # noqa: F401
 from .tree import ancestor_chains, tree_mask, sequence_expanded_attention  # noqa: F401
 from .replay import replay_step_attention, replay_beam_attention  # noqa: F401
 from .brute_force import enumerate_all_paths  # noqa: F401
+from .encdec import (  # noqa: F401
+    cross_attention, target_attention, self_tree_attention, cross_plus_self_attention, path_hidden_states,
+)

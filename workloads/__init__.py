@@ -11,7 +11,7 @@ here is a seeded draw with the shape and structure of the paper's workload
 (one long shared user history, d = 3-4 SID levels, per-level codebook, wide
 beam, GQA 4:1 — PAPER.md:126, 138, 304, 306).
 """
-from .configs import StarkConfig, CONFIGS, get_config, beam_widths, queries_per_step  # noqa: F401
+from .configs import StarkConfig, CONFIGS, N_FIXED, get_config, beam_widths, queries_per_step  # noqa: F401
 from .generate import (  # noqa: F401
     rng_for,
     round_to_bf16,
@@ -23,4 +23,6 @@ from .generate import (  # noqa: F401
     step_logits,
     config1_tables,
     tie_logits,
+    fixed_prefix_kv,
+    step_q_cross,
 )

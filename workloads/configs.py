@@ -109,5 +109,14 @@ F32_GQA = _add(replace(CFG1, name="f32_gqa", config_id=27, B=3, Hq=8, Hkv=2,
                        kv_std=1.0, q_std=1.0, logits="normal"))
 
 
+# --- the paper's encoder-decoder form (readings R23-R25): `prefix_*` is the length of
+# the encoder memory M; the decoder's own fixed prefix [e_click, e_atc, e_pay, <bos>]
+# (Eq. 7) has 4 rows per user.  cfg2's heads / memory length / beam / codebook.
+ENCDEC = _add(replace(CFG2, name="encdec", config_id=31))
+ENCDEC_S = _add(replace(CFG2, name="encdec_small", config_id=32, B=3, prefix_min=150, prefix_max=333,
+                        W=(24, 24, 24), C=48))
+N_FIXED = 4   # e_click, e_atc, e_pay, <bos>
+
+
 def get_config(name: str) -> StarkConfig:
     return CONFIGS[name]

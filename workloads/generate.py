@@ -18,7 +18,7 @@ import numpy as np
 from .configs import StarkConfig
 
 # RNG stream tags
-_T_LEN, _T_PREFIX, _T_SCALE, _T_STEP, _T_LOGITS, _T_TABLES = 1, 2, 3, 4, 5, 6
+_T_LEN, _T_PREFIX, _T_SCALE, _T_STEP, _T_LOGITS, _T_TABLES, _T_FIXED, _T_QCROSS = 1, 2, 3, 4, 5, 6, 7, 8
 
 
 def rng_for(seed: int, cfg: StarkConfig, tag: int, *idx: int) -> np.random.Generator:
@@ -121,6 +121,25 @@ def step_logits(cfg: StarkConfig, t: int, n_q: int, seed: int = 0,
         else:
             out[j] = g.standard_normal((n_q, cfg.C), dtype=np.float32) * np.float32(cfg.logits_std)
     return out
+
+
+def fixed_prefix_kv(cfg: StarkConfig, seed: int = 0, n_fixed: int = 4) -> Tuple[np.ndarray, np.ndarray]:
+    """Encoder-decoder form: self-attention K, V of the decoder's fixed prefix positions
+    [e_click, e_atc, e_pay, <bos>] (Eq. 7), per user: [B, n_fixed, Hkv, D] ~ N(0, kv_std)."""
+    g = rng_for(seed, cfg, _T_FIXED)
+    k = g.standard_normal((cfg.B, n_fixed, cfg.Hkv, cfg.D), dtype=np.float32) * np.float32(cfg.kv_std)
+    v = g.standard_normal((cfg.B, n_fixed, cfg.Hkv, cfg.D), dtype=np.float32) * np.float32(cfg.kv_std)
+    return _finish(k, cfg), _finish(v, cfg)
+
+
+def step_q_cross(cfg: StarkConfig, t: int, n_q: int, seed: int = 0) -> np.ndarray:
+    """Encoder-decoder form: the cross-attention queries of step t (a projection of their own):
+    [B, n_q, Hq, D] ~ N(0, q_std), fresh draws per (step, user, slot) like step_qkv."""
+    out = np.empty((cfg.B, n_q, cfg.Hq, cfg.D), dtype=np.float32)
+    for u in range(cfg.B):
+        g = rng_for(seed, cfg, _T_QCROSS, t, u)
+        out[u] = g.standard_normal((n_q, cfg.Hq, cfg.D), dtype=np.float32) * np.float32(cfg.q_std)
+    return _finish(out, cfg)
 
 
 def tie_logits(logits: np.ndarray) -> np.ndarray:
