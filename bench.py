@@ -11,7 +11,8 @@ metric = generated SIDs/s (B * W_d final beams per pass / pass time); also us pe
 
 Headline workload: cfg5 (BASELINE.json configs[4], the largest single-GPU configuration; BASELINE.json's metric
 names no configuration).  The same JSON line carries `per_config`: cfg1, cfg2, cfg3 (attention-side shape), cfg4,
-paper_b8, paper_b1 -- pass time (median and min over >= 100 graph replays), SIDs/s and a per-kernel table (fused
+paper_b8, paper_b1, encdec (the paper's encoder-decoder form) -- pass time (median and min over >= 100 graph
+replays), SIDs/s and a per-kernel table (fused
 launches AND the four north-star calls as separate launches) with roofline fractions against the measured and
 the nominal peaks.
 
@@ -40,7 +41,7 @@ L2_BYTES = 126 * 2 ** 20
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 NOMINAL = {"hbm_gbs": 8000.0, "bf16_tflops": 2250.0}     # north star "~8 TB/s"; vendor dense bf16
 HEADLINE = "cfg5"
-PER_CONFIG = ["cfg1", "cfg2", "cfg3", "cfg4", "paper_b8", "paper_b1"]
+PER_CONFIG = ["cfg1", "cfg2", "cfg3", "cfg4", "paper_b8", "paper_b1", "encdec"]
 
 
 def parse_args():
@@ -605,6 +606,74 @@ def measure_config(torch, cfg, dev, pk, args, replays=100):
     return ent
 
 
+def measure_encdec(torch, cfg, dev, pk, args, replays=100):
+    """`per_config` entry of the paper's encoder-decoder form (pipeline.EncDecPass): per
+    decode step cross-attention over the memory M (stark_decode_attn, level 0), self-attention over the 4 fixed
+    decoder positions + chain (stark_decode_step), stark_beam_topk."""
+    from paper_2607_04068_b200.pipeline import EncDecPass
+    t_in = time.perf_counter()
+    up = lambda a, d=None: (torch.from_numpy(a).to(dev).to(d) if d is not None else torch.from_numpy(a).to(dev)).contiguous()
+    bf = torch.bfloat16
+    nq, widths, d = wl.queries_per_step(cfg), wl.beam_widths(cfg), cfg.d
+    eb = cfg.elem_bytes
+
+    def one(seed):
+        K, V, cu = wl.prefix_kv(cfg, seed)
+        Kf, Vf = wl.fixed_prefix_kv(cfg, seed)
+        q, k, v, qc, lg = [], [], [], [], []
+        for t in range(d):
+            qq, kk, vv = wl.step_qkv(cfg, t, nq[t], seed)
+            q.append(up(qq, bf)), k.append(up(kk, bf)), v.append(up(vv, bf)), qc.append(up(wl.step_q_cross(cfg, t, nq[t], seed), bf))
+            lg.append(torch.log_softmax(up(wl.step_logits(cfg, t, nq[t], seed)), dim=-1).contiguous())
+        lens = np.diff(cu)
+        nbytes = (K.size + V.size) * eb + sum(x.numel() * x.element_size() for x in q + k + v + qc + lg)
+        return EncDecPass(cfg.B, cfg.Hq, cfg.Hkv, cfg.D, d, cfg.C, widths, bf, up(K, bf), up(V, bf), up(cu.astype(np.int32)),
+                          int(lens.max()), up(Kf, bf), up(Vf, bf), qc, q, k, v, lg), lens, nbytes
+
+    p0, lens, set_bytes = one(0)
+    R = args.sets or int(min(16, max(2, -(-2 * L2_BYTES // set_bytes))))
+    passes = [p0] + [one(r)[0] for r in range(1, R)]
+    use_graph = not args.no_graph
+    calls, call_all = capture_passes(torch, passes, use_graph)
+    med, mn, mean = replay_stats(torch, call_all, R, replays)
+    kern = {}
+
+    def put(name, fns, byts, flops=None):
+        m, lo = time_graph_loop(torch, fns, 240, use_graph, stats=True)
+        kern[name] = {"us": m, "us_min": lo, "bytes": byts} | ({"flops": flops} if flops is not None else {})
+
+    fixed = np.full(cfg.B, EncDecPass.N_FIXED)
+    for t in range(d):
+        fl, by = work_decode(cfg, lens, nq[t], 0)
+        put(f"cross_attn.t{t}", [(lambda p=p, t=t: p.mem.attend(0, p.q_cross[t], out=p.cross[t], fused=True)) for p in passes], by, fl)
+        fl, by = work_decode(cfg, fixed, nq[t], t)
+        put(f"self_attn_step.t{t}", [(lambda p=p, t=t: p.dec.step(t, p.q_self[t], p.k_new[t] if t else None, p.v_new[t] if t else None,
+                                                                 p.sel[t - 1][1] if t else None, out=p.self_out[t])) for p in passes],
+            by + (work_append(cfg, nq[t]) if t else 0), fl)
+        put(f"beam_topk.t{t}", [(lambda p=p, t=t: __import__("paper_2607_04068_b200.decode", fromlist=["beam_topk"]).beam_topk(
+            p.logp[t], p.sel[t - 1][0] if t else None, p.widths[t], out=p.sel[t], ws=p.topk_ws)) for p in passes],
+            work_topk(cfg, nq[t], widths[t]))
+    hbm, tfl = pk["hbm_gbs"], pk["bf16_tflops"]
+    for v in kern.values():
+        v["GBps"] = v["bytes"] / v["us"] * 1e-3
+        fl = v.get("flops", 0.0)
+        t_h, t_t = v["bytes"] / (hbm * 1e3), fl / (tfl * 1e6)
+        v["roofline_us"], v["bound"] = max(t_h, t_t), ("tensor" if t_t > t_h else "hbm")
+        v["frac"] = v["roofline_us"] / v["us"]
+        v["frac_nominal"] = max(v["bytes"] / (NOMINAL["hbm_gbs"] * 1e3), fl / (NOMINAL["bf16_tflops"] * 1e6)) / v["us"]
+    ent = {"pass_us_median": med, "pass_us_min": mn, "pass_us_mean": mean, "replays": replays, "passes_per_replay": R,
+           "sids_per_s": cfg.B * widths[-1] / (med * 1e-6), "us_per_decode_step": med / d, "launches_per_pass": 3 * d,
+           "dtype": cfg.dtype, "form": "encoder-decoder: cross-attention over M + self-attention over [TAT, bos] + chain, two softmaxes",
+           "shape": {"B": cfg.B, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D, "memory_len": [int(lens.min()), int(lens.max())],
+                     "fixed_decoder_positions": EncDecPass.N_FIXED, "beam": list(widths), "levels": d, "codebook": cfg.C},
+           "l2": f"{R} rotating input sets ({R * set_bytes / 2**20:.0f} MiB)",
+           "kernel_sum_us": sum(v["us"] for v in kern.values()), "kernels": rnd(kern)}
+    del passes, calls, call_all, p0
+    torch.cuda.empty_cache()
+    ent["bench_wall_s"] = round(time.perf_counter() - t_in, 1)
+    return ent
+
+
 def run_stark(args, cfg):
     import torch
     import torch.distributed as dist
@@ -812,7 +881,7 @@ def run_stark(args, cfg):
         per = {}
         for n in names:
             try:
-                per[n] = measure_config(torch, wl.get_config(n), dev, pk, args)
+                per[n] = (measure_encdec if n.startswith("encdec") else measure_config)(torch, wl.get_config(n), dev, pk, args)
             except Exception as e:  # noqa: BLE001  (one config failing must not lose the headline)
                 per[n] = {"error": repr(e)}
         line["per_config"] = per

@@ -82,3 +82,49 @@ class DecodePass:
             cols[t] = torch.gather(self.sel[t][2].long(), 1, slot)
             slot = torch.gather(self.sel[t][1].long(), 1, slot)
         return torch.stack(cols, dim=2)
+
+
+class EncDecPass:
+    """One pass of the hot path in the paper's ENCODER-DECODER form (DESIGN.md
+    readings R23-R25): per decode step t two attention sub-layers instead of one --
+      * cross-attention over the encoder memory M: the shared-prefix partials finalised ALONE
+        (stark_decode_attn at level 0: every beam of a user attends the same M, read once per step);
+      * causal self-attention over [e_click, e_atc, e_pay, <bos>] + the beam's ancestor chain (Eq. 7 and Eq. 14,
+        PAPER.md:197-204, 265-268): the same library with a 4-row "prefix" per user (stark_decode_step: the
+        level's K/V append rides inside the launch);
+    then stark_beam_topk.  `run()` only enqueues library calls (CUDA-graph capturable)."""
+
+    N_FIXED = 4
+
+    def __init__(self, B: int, Hq: int, Hkv: int, D: int, d: int, C: int, widths: List[int], dtype: torch.dtype,
+                 k_mem: torch.Tensor, v_mem: torch.Tensor, cu_mem: torch.Tensor, max_mem_len: int,
+                 k_fix: torch.Tensor, v_fix: torch.Tensor, q_cross: List[torch.Tensor], q_self: List[torch.Tensor],
+                 k_new: List[torch.Tensor], v_new: List[torch.Tensor], logp: List[torch.Tensor]):
+        assert dtype == torch.bfloat16, "the fused launches are bf16 (fp32: compose stark_prefix_attn + stark_tree_attn_step)"
+        self.B, self.d, self.C, self.widths = B, d, C, list(widths)
+        self.n_q = [1] + self.widths
+        dev = k_mem.device
+        Wmax = max(self.widths)
+        self.mem = StarkLayer(B, Hq, Hkv, D, d, Wmax, dtype, k_mem, v_mem, cu_mem, max_mem_len)
+        cu_fix = (torch.arange(B + 1, device=dev, dtype=torch.int32) * self.N_FIXED).contiguous()
+        self.dec = StarkLayer(B, Hq, Hkv, D, d, Wmax, dtype, k_fix.reshape(B * self.N_FIXED, Hkv, D).contiguous(),
+                              v_fix.reshape(B * self.N_FIXED, Hkv, D).contiguous(), cu_fix, self.N_FIXED)
+        self.q_cross, self.q_self, self.k_new, self.v_new, self.logp = q_cross, q_self, k_new, v_new, logp
+        shp = sb.make_shape(B, 1, 1, 64, 1, max(self.n_q), torch.float32)
+        need = max(sb.stark_workspace_bytes(shp, sb.CALL_BEAM_TOPK, self.n_q[t], C) for t in range(d))
+        self.topk_ws = torch.zeros(need, dtype=torch.uint8, device=dev) if need else None
+        self.cross = [torch.empty_like(q_cross[t]) for t in range(d)]
+        self.self_out = [torch.empty_like(q_self[t]) for t in range(d)]
+        self.sel = [(torch.empty((B, w), dtype=torch.float32, device=dev),
+                     torch.empty((B, w), dtype=torch.int32, device=dev),
+                     torch.empty((B, w), dtype=torch.int32, device=dev)) for w in self.widths]
+
+    launches = property(lambda self: 3 * self.d)
+
+    def run(self) -> None:
+        score = parent = None
+        for t in range(self.d):
+            self.mem.attend(0, self.q_cross[t], out=self.cross[t], fused=True)
+            self.dec.step(t, self.q_self[t], self.k_new[t] if t >= 1 else None, self.v_new[t] if t >= 1 else None,
+                          parent, out=self.self_out[t])
+            score, parent, _ = beam_topk(self.logp[t], score, self.widths[t], out=self.sel[t], ws=self.topk_ws)
