@@ -223,6 +223,13 @@ __device__ __forceinline__ void st_cluster_f2(uint32_t addr, float a, float b) {
     asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
 }
 
+#ifdef STARK_TC_PROF   // per-iteration timeline of ONE CTA (scratch builds only; never defined in the product build)
+__device__ long long g_tc_prof[64 * 16];
+#define TCPROF(j, slot) do { if ((j) < 64 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == STARK_TC_PROF) g_tc_prof[(j) * 16 + (slot)] = clock64(); } while (0)
+#else
+#define TCPROF(j, slot) do {} while (0)
+#endif
+
 template <int D> struct TcCfg {
     static constexpr int BOXES = D / 64;                 // 64-element (128-byte) column boxes per row
     static constexpr int TILE_BYTES = BOXES * BM * 128;  // one 128-row tile of Q, K or V
@@ -595,13 +602,17 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 umma_commit(bar_empty + 8 * slot_of(0));
                 for (int j = 0; j < n_tiles; ++j) {
                     const bool more = j + 1 < n_tiles;
+                    TCPROF(j, 13);
                     wait_full(2 * j + 1);                    // V_j
                     if (more) wait_full(2 * j + 2);          // K_{j+1}
+                    TCPROF(j, 12);
                     for (int t = 0; t < nt; ++t) {
                         mbar_wait(bar_pfull + 8 * t, (uint32_t)(j & 1));
                         tc_fence_after();
+                        TCPROF(j, 8 + 2 * t);
                         issue_pv(t, slot_of(2 * j + 1), j > 0);
                         if (more) issue_qk(t, slot_of(2 * j + 2));
+                        TCPROF(j, 9 + 2 * t);
                     }
                     umma_commit(bar_empty + 8 * slot_of(2 * j + 1));
                     if (more) umma_commit(bar_empty + 8 * slot_of(2 * j + 2));
@@ -674,8 +685,10 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
             const uint32_t aS = lane_addr + C::COL_S + t * BN;
             const int my_tiles = parity ? (n_tiles - t + 1) / 2 : n_tiles;  // KV tiles of this accumulator set
             for (int j = 0; j < my_tiles; ++j) {
+                if (quarter == 0 && lane == 0) TCPROF(j, 4 * t + 0);
                 mbar_wait(bar_sfull + 8 * t, (uint32_t)(j & 1));
                 __syncwarp();
+                if (quarter == 0 && lane == 0) TCPROF(j, 4 * t + 1);
                 if (warp_live) {                        // warps without live rows only keep the barrier count
                     tc_fence_after();
                     const int x = parity ? 2 * j + t : j;            // KV tile of the split
@@ -685,6 +698,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
 #pragma unroll
                     for (int c = 0; c < 4; ++c) tmem_ld32(aS + c * 32, sr[c]);
                     tmem_wait_ld();
+                    if (quarter == 0 && lane == 0) TCPROF(j, 4 * t + 2);
                     if (valid < BN) {
 #pragma unroll
                         for (int c = 0; c < 4; ++c)
@@ -746,6 +760,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                     l_sum += ps0 + ps1;
                     tmem_wait_st();
                     tc_fence_before();
+                    if (quarter == 0 && lane == 0) TCPROF(j, 4 * t + 3);
                 }
                 mbar_arrive(bar_pfull + 8 * t);
             }
@@ -1046,3 +1061,9 @@ int launch_decode_fused(const Dims& p, const void* q, int n_q, int level, const 
 }
 
 }  // namespace stark
+
+#ifdef STARK_TC_PROF
+extern "C" int stark_debug_tc_prof(long long* host_out) {
+    return (int)cudaMemcpyFromSymbol(host_out, stark::g_tc_prof, sizeof(stark::g_tc_prof));
+}
+#endif
