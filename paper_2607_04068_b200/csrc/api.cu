@@ -196,7 +196,7 @@ int stark_prefix_attn(const stark_shape_t* shape, const void* q, int n_q, const 
     if (n_splits == 0) n_splits = plan_splits(p, shape->dtype, n_q, max_prefix_len);
     cudaStream_t st = (cudaStream_t)stream;
     if (prefix_tc_supported(p, shape->dtype, n_q))
-        return launch_prefix_tc(p, q, n_q, k_prefix, v_prefix, cu_seqlens, total_tokens, n_splits, part_m,
+        return launch_prefix_tc(p, q, n_q, k_prefix, v_prefix, cu_seqlens, total_tokens, max_prefix_len, n_splits, part_m,
                                 part_l, part_o, st);
     return launch_prefix_simt(p, shape->dtype, q, n_q, k_prefix, v_prefix, cu_seqlens, n_splits, part_m,
                               part_l, part_o, st);
@@ -231,7 +231,7 @@ int stark_decode_attn(const stark_shape_t* shape, const void* q, int n_q, int le
     rc = check_device();
     if (rc != STARK_OK) return rc;
     const int32_t* anc_l = anc ? anc + (size_t)(level & 1) * p.B * p.Wmax * p.d : nullptr;
-    return launch_decode_fused(p, q, n_q, level, k_prefix, v_prefix, cu_seqlens, total_tokens,
+    return launch_decode_fused(p, q, n_q, level, k_prefix, v_prefix, cu_seqlens, total_tokens, max_prefix_len,
                                plan_cluster_splits(p, n_q, max_prefix_len), k_suffix, v_suffix, anc_l, out,
                                (cudaStream_t)stream);
 }
@@ -254,7 +254,7 @@ int stark_decode_step(const stark_shape_t* shape, const void* q, int n_q, int le
     const size_t half = (size_t)p.B * p.Wmax * p.d;
     const int32_t* anc_prev = level >= 1 ? anc + (size_t)((level - 1) & 1) * half : nullptr;
     int32_t* anc_new = (level >= 1 && write_anc) ? anc + (size_t)(level & 1) * half : nullptr;
-    return launch_decode_fused(p, q, n_q, level, k_prefix, v_prefix, cu_seqlens, total_tokens,
+    return launch_decode_fused(p, q, n_q, level, k_prefix, v_prefix, cu_seqlens, total_tokens, max_prefix_len,
                                plan_cluster_splits(p, n_q, max_prefix_len), k_suffix, v_suffix, anc_prev, out,
                                (cudaStream_t)stream, level >= 1 ? k_new : nullptr, level >= 1 ? v_new : nullptr, parent,
                                anc_new);

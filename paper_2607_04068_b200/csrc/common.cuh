@@ -101,12 +101,12 @@ int launch_prefix_simt(const Dims& p, int dtype, const void* q, int n_q, const v
                        cudaStream_t st);
 // returns STARK_ERR_UNSUPPORTED when the shape has no tensor-core path
 int launch_prefix_tc(const Dims& p, const void* q, int n_q, const void* k, const void* v,
-                     const int32_t* cu, int total_tokens, int n_splits, float* pm, float* pl,
+                     const int32_t* cu, int total_tokens, int max_len, int n_splits, float* pm, float* pl,
                      float* po, cudaStream_t st);
 bool prefix_tc_supported(const Dims& p, int dtype, int n_q);
 bool prefix_tc_parity(const Dims& p, int n_q, int n_splits);
 int launch_decode_fused(const Dims& p, const void* q, int n_q, int level, const void* k, const void* v,
-                        const int32_t* cu, int total_tokens, int n_splits, const void* ks, const void* vs,
+                        const int32_t* cu, int total_tokens, int max_len, int n_splits, const void* ks, const void* vs,
                         const int32_t* anc_level, void* out, cudaStream_t st, const void* kn = nullptr,
                         const void* vn = nullptr, const int32_t* parent = nullptr, int32_t* anc_new = nullptr);
 int launch_tree_attn(const Dims& p, int dtype, const void* q, int n_q, int level, const void* ks,

@@ -422,7 +422,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1)
 prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                  const __grid_constant__ CUtensorMap tm_v, const int32_t* __restrict__ cu,
                  float* __restrict__ pm, float* __restrict__ pl, float* __restrict__ po, int B, int n_q,
-                 int Hq, int Hkv, int G, int n_splits, float scale_log2, int parity, const FusedArgs fa) {
+                 int Hq, int Hkv, int G, int n_splits, float scale_log2, int parity, int lpt, const FusedArgs fa) {
     // Two TMEM accumulator sets (S_t/P_t, O_t), t = 0, 1, each served by its own softmax warpgroup:
     //   pair mode   (parity = 0): the CTA owns Q tiles 2x and 2x+1; set t = Q tile t; both see every KV tile.
     //   parity mode (parity = 1): the CTA owns ONE Q tile; set t = the KV tiles of parity t (two independent
@@ -434,8 +434,28 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     // FUSED: the splits of one KV head are adjacent in y (cluster dims (1, n_splits, 1))
     const int kv = FUSED ? blockIdx.y / n_splits : blockIdx.y % Hkv;
     const int split = FUSED ? blockIdx.y % n_splits : blockIdx.y / Hkv;
-    const int u = blockIdx.z;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int u = blockIdx.z;
+    if (lpt) {
+        // Ragged batch (B <= 64): CTAs are handed out in grid order, so the users are taken LONGEST PREFIX FIRST
+        // (blockIdx.z = rank by length, ties by index): a long user started last would run alone at the end
+        // (measured at config 5, lengths 1.2-8.2 K: SMs idle 8 % of the kernel).
+        __shared__ int s_user;
+        if (warp == 0) {
+            const int l0 = lane < B ? cu[lane + 1] - cu[lane] : -1;
+            const int l1 = lane + 32 < B ? cu[lane + 33] - cu[lane + 32] : -1;
+            int rk0 = 0, rk1 = 0;
+            for (int k = 0; k < B; ++k) {
+                const int lk = __shfl_sync(0xffffffffu, k < 32 ? l0 : l1, k & 31);
+                rk0 += (lk > l0 || (lk == l0 && k < lane)) ? 1 : 0;
+                rk1 += (lk > l1 || (lk == l1 && k < lane + 32)) ? 1 : 0;
+            }
+            if (lane < B && rk0 == (int)blockIdx.z) s_user = lane;
+            if (lane + 32 < B && rk1 == (int)blockIdx.z) s_user = lane + 32;
+        }
+        __syncthreads();
+        u = s_user;
+    }
 
     const int row_begin = cu[u];
     const int L = cu[u + 1] - row_begin;
@@ -511,7 +531,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_v) : "memory");
         mbar_init(bar_q, 1);
         for (int s = 0; s < NS; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
-        for (int t = 0; t < 2; ++t) { mbar_init(bar_sfull + 8 * t, 1); mbar_init(bar_pfull + 8 * t, kSoftmaxThreads); }
+        for (int t = 0; t < 2; ++t) { mbar_init(bar_sfull + 8 * t, 1); mbar_init(bar_pfull + 8 * t, kSoftmaxThreads / 32); }
         mbar_init(bar_done, 1);
         fence_barrier_init();
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -693,31 +713,41 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                     tc_fence_after();
                     const int x = parity ? 2 * j + t : j;            // KV tile of the split
                     const int valid = min(BN, r1 - (r0 + x * BN));   // columns of this tile inside the split
-                    // the whole S row (128 fp32) into registers with one wait, then its maximum
+                    // the whole S row (128 fp32) into registers; the maximum of its first half is taken while
+                    // the second half is still on its way from TMEM
                     uint32_t sr[4][32];
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) tmem_ld32(aS + c * 32, sr[c]);
+                    tmem_ld32(aS, sr[0]);
+                    tmem_ld32(aS + 32, sr[1]);
                     tmem_wait_ld();
+                    tmem_ld32(aS + 64, sr[2]);
+                    tmem_ld32(aS + 96, sr[3]);
                     if (quarter == 0 && lane == 0) TCPROF(j, 4 * t + 2);
-                    if (valid < BN) {
-#pragma unroll
-                        for (int c = 0; c < 4; ++c)
-#pragma unroll
-                            for (int x = 0; x < 32; ++x)
-                                if (c * 32 + x >= valid) sr[c][x] = 0xff800000u;  // -inf: exp2 gives exactly 0
-                    }
                     // 4 independent running maxima: with two warps per scheduler a single 128-long dependent
                     // chain (4 cycles per link) would cost as much as the exponentials themselves
                     float tm0 = -INFINITY, tm1 = -INFINITY, tm2 = -INFINITY, tm3 = -INFINITY;
+                    auto max_half = [&](int c0) {
 #pragma unroll
-                    for (int c = 0; c < 4; ++c)
+                        for (int c = c0; c < c0 + 2; ++c)
 #pragma unroll
-                        for (int x = 0; x < 32; x += 4) {
-                            tm0 = fmaxf(tm0, __uint_as_float(sr[c][x]));
-                            tm1 = fmaxf(tm1, __uint_as_float(sr[c][x + 1]));
-                            tm2 = fmaxf(tm2, __uint_as_float(sr[c][x + 2]));
-                            tm3 = fmaxf(tm3, __uint_as_float(sr[c][x + 3]));
-                        }
+                            for (int x = 0; x < 32; x += 4) {
+                                tm0 = fmaxf(tm0, __uint_as_float(sr[c][x]));
+                                tm1 = fmaxf(tm1, __uint_as_float(sr[c][x + 1]));
+                                tm2 = fmaxf(tm2, __uint_as_float(sr[c][x + 2]));
+                                tm3 = fmaxf(tm3, __uint_as_float(sr[c][x + 3]));
+                            }
+                    };
+                    auto mask_half = [&](int c0) {              // columns beyond the split: -inf (exp2 gives 0)
+#pragma unroll
+                        for (int c = c0; c < c0 + 2; ++c)
+#pragma unroll
+                            for (int x = 0; x < 32; ++x)
+                                if (c * 32 + x >= valid) sr[c][x] = 0xff800000u;
+                    };
+                    if (valid < BN) mask_half(0);
+                    max_half(0);
+                    tmem_wait_ld();
+                    if (valid < BN) mask_half(2);
+                    max_half(2);
                     float tmax = fmaxf(fmaxf(tm0, tm1), fmaxf(tm2, tm3));
                     tmax *= scale_log2;
                     // lazy rescale: keep the reference maximum unless the row maximum grew by > 2^8
@@ -762,7 +792,8 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                     tc_fence_before();
                     if (quarter == 0 && lane == 0) TCPROF(j, 4 * t + 3);
                 }
-                mbar_arrive(bar_pfull + 8 * t);
+                __syncwarp();                           // every lane's P is written and fenced: one arrival per warp
+                if (lane == 0) mbar_arrive(bar_pfull + 8 * t);
             }
             // ---- epilogue: O row -> partials ----
             if (FUSED && vpre) {
@@ -964,7 +995,7 @@ bool make_map(CUtensorMap* tm, const void* base, int D, int n1, long long n2, in
 
 template <int D>
 int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, int n_q,
-             const int32_t* cu, int n_splits, float* pm, float* pl, float* po, cudaStream_t st) {
+             const int32_t* cu, int n_splits, int lpt, float* pm, float* pl, float* po, cudaStream_t st) {
     static PerDevice<bool> attr_done;
     if (!attr_done.here()) {
         STARK_CUDA_TRY(cudaFuncSetAttribute(prefix_tc_kernel<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -976,7 +1007,7 @@ int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const 
     const int rows_per_cta = parity ? BM : 2 * BM;                  // one Q tile, or a pair of them
     dim3 grid((M + rows_per_cta - 1) / rows_per_cta, p.Hkv * n_splits, p.B);
     prefix_tc_kernel<D, false><<<grid, kThreadsTC, TcCfg<D>::SMEM_BYTES, st>>>(
-        tq, tk, tv, cu, pm, pl, po, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits, p.scale * kLog2e, parity, FusedArgs{});
+        tq, tk, tv, cu, pm, pl, po, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits, p.scale * kLog2e, parity, lpt, FusedArgs{});
     STARK_LAUNCH_CHECK();
     return STARK_OK;
 }
@@ -984,7 +1015,7 @@ int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const 
 // fused launch: the n_splits CTAs of one (pair, KV head, user) are a cluster along y
 template <int D>
 int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, int n_q,
-                   const int32_t* cu, int n_splits, const FusedArgs& fa, cudaStream_t st) {
+                   const int32_t* cu, int n_splits, int lpt, const FusedArgs& fa, cudaStream_t st) {
     static PerDevice<bool> attr_done;
     if (!attr_done.here()) {
         STARK_CUDA_TRY(cudaFuncSetAttribute(prefix_tc_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -1005,7 +1036,7 @@ int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, 
     cfg.attrs = at; cfg.numAttrs = n_splits > 1 ? 1 : 0;   // a single split needs no cluster launch
     STARK_CUDA_TRY(cudaLaunchKernelEx(&cfg, prefix_tc_kernel<D, true>, tq, tk, tv, cu, (float*)nullptr,
                                       (float*)nullptr, (float*)nullptr, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits,
-                                      p.scale * kLog2e, parity, fa));
+                                      p.scale * kLog2e, parity, lpt, fa));
     return STARK_OK;
 }
 
@@ -1019,6 +1050,11 @@ bool prefix_tc_parity(const Dims& p, int n_q, int n_splits) {
     return tiles_m * p.Hkv * p.B * n_splits <= sms;
 }
 
+// Longest-prefix-first CTA order pays only for ragged batches; the kernel's ranking handles up to 64 users.
+static int ragged_batch(const Dims& p, int total_tokens, int max_len) {
+    return (p.B >= 2 && p.B <= 64 && (long long)max_len * p.B != (long long)total_tokens) ? 1 : 0;
+}
+
 bool prefix_tc_supported(const Dims& p, int dtype, int n_q) {
     if (dtype != STARK_BF16) return false;
     if (p.D != 64 && p.D != 128) return false;
@@ -1027,7 +1063,7 @@ bool prefix_tc_supported(const Dims& p, int dtype, int n_q) {
 }
 
 int launch_prefix_tc(const Dims& p, const void* q, int n_q, const void* k, const void* v, const int32_t* cu,
-                     int total_tokens, int n_splits, float* pm, float* pl, float* po, cudaStream_t st) {
+                     int total_tokens, int max_len, int n_splits, float* pm, float* pl, float* po, cudaStream_t st) {
     if (total_tokens < 1)
         return launch_prefix_simt(p, STARK_BF16, q, n_q, k, v, cu, n_splits, pm, pl, po, st);
     CUtensorMap tq, tk, tv;
@@ -1036,13 +1072,14 @@ int launch_prefix_tc(const Dims& p, const void* q, int n_q, const void* k, const
         last_cuda_error_ref() = (int)cudaErrorInvalidValue;
         return STARK_ERR_CUDA;
     }
-    if (p.D == 128) return launch_d<128>(p, tq, tk, tv, n_q, cu, n_splits, pm, pl, po, st);
-    return launch_d<64>(p, tq, tk, tv, n_q, cu, n_splits, pm, pl, po, st);
+    const int lpt = ragged_batch(p, total_tokens, max_len);
+    if (p.D == 128) return launch_d<128>(p, tq, tk, tv, n_q, cu, n_splits, lpt, pm, pl, po, st);
+    return launch_d<64>(p, tq, tk, tv, n_q, cu, n_splits, lpt, pm, pl, po, st);
 }
 
 // A1 + A2 in one launch (bf16): n_splits in {1, 2, 4, 8} = cluster size along the prefix.
 int launch_decode_fused(const Dims& p, const void* q, int n_q, int level, const void* k, const void* v,
-                        const int32_t* cu, int total_tokens, int n_splits, const void* ks, const void* vs,
+                        const int32_t* cu, int total_tokens, int max_len, int n_splits, const void* ks, const void* vs,
                         const int32_t* anc_level, void* out, cudaStream_t st, const void* kn, const void* vn,
                         const int32_t* parent, int32_t* anc_new) {
     CUtensorMap tq, tk, tv;
@@ -1056,8 +1093,9 @@ int launch_decode_fused(const Dims& p, const void* q, int n_q, int level, const 
     fa.anc = anc_level; fa.out = (__nv_bfloat16*)out;
     fa.level = level; fa.Wmax = p.Wmax; fa.d = p.d; fa.scale = p.scale;
     fa.kn = (const __nv_bfloat16*)kn; fa.vn = (const __nv_bfloat16*)vn; fa.parent = parent; fa.anc_new = anc_new;
-    if (p.D == 128) return launch_fused_d<128>(p, tq, tk, tv, n_q, cu, n_splits, fa, st);
-    return launch_fused_d<64>(p, tq, tk, tv, n_q, cu, n_splits, fa, st);
+    const int lpt = ragged_batch(p, total_tokens, max_len);
+    if (p.D == 128) return launch_fused_d<128>(p, tq, tk, tv, n_q, cu, n_splits, lpt, fa, st);
+    return launch_fused_d<64>(p, tq, tk, tv, n_q, cu, n_splits, lpt, fa, st);
 }
 
 }  // namespace stark
