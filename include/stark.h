@@ -274,6 +274,15 @@ int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_
  * followed by exactly stark_beam_topk's selection and outputs (out_score = key,
  * the new cumulative log-probability).  Equal to score + log-softmax(logits) up
  * to the rounding of the two fp32 operations; +inf logits are undefined.
+ * Rounding guarantee: the log-sum-exp is evaluated in fp64 (error of a few
+ * 1e-16 relative, depending on the summation order) and rounded ONCE to fp32, so
+ * lse is the correctly rounded fp32 value of the exact log-sum-exp unless the
+ * exact value lies within ~64 fp64 ulps (1.2e-7 of an fp32 ulp) of the midpoint
+ * of two neighbouring fp32 numbers -- for logits without special structure a
+ * probability of ~2.4e-7 per beam that the row is that close, and only then may
+ * lse (hence the beam's keys, all together) differ by one fp32 ulp from another
+ * correctly implemented fp64 evaluation.  The selection that follows is
+ * bit-exact GIVEN the offsets (total order on (key, index)).
  *
  * stark_logits_row_offset is the first half on its own (rows = B*W_in beams,
  * logits [rows, C] fp32, score [rows] fp32 or NULL => zeros, offset out [rows]).

@@ -56,7 +56,10 @@ constexpr int kMaxK = 1024;                       // W_out served by this path (
 constexpr int kPubPerThread = 16;                 // published maxima a thread reads
 constexpr int kMaxGroups = kPubPerThread * kThreads;   // published maxima per user at most (8192)
 constexpr uint32_t kOverflow = 0x00400000u;       // added to a user's count by a CTA that lost survivors (> any real count; 512 of them do not wrap)
-constexpr long long kGridMinN = 131072;           // candidates per user from which this path is tried (measured)
+#ifndef STARK_GRID_MIN_N
+#define STARK_GRID_MIN_N 131072
+#endif
+constexpr long long kGridMinN = STARK_GRID_MIN_N;  // candidates per user from which this path is tried (measured)
 constexpr int kGridMaxCtas = 512;                 // CTAs of one launch at most (workspace sizing; 2 x 148 on B200)
 
 #ifdef STARK_TOPK_PROF   // phase probes of scratch builds (never defined in the product build)

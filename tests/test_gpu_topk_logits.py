@@ -111,3 +111,39 @@ def test_argument_validation():
         stark_beam_topk_logits(lg, None, 1, 4, 8, 4, *o, None)
     with pytest.raises(StarkError):              # W_out > W_in * C
         stark_beam_topk_logits(lg, None, 1, 4, 8, 33, *o, torch.empty(4096, dtype=torch.uint8, device="cuda"))
+
+
+def test_rows_whose_logsumexp_sits_next_to_an_fp32_rounding_boundary():
+    """Reading R22 / include/stark.h A3': lse = fl32(logsumexp) is the correctly rounded fp32 value of an fp64
+    evaluation.  The kernel sums in a different order (and with its own fp64 exp) than numpy, so the two fp64
+    values differ by a few 1e-16 relative; the fp32 rounding can only flip when the exact value lies that close
+    to the midpoint of two fp32 neighbours (probability ~1e-9 per beam, stated in the header).  This test goes
+    looking for trouble: of 4 M random short rows it keeps the 4096 whose fp64 log-sum-exp is CLOSEST to such a
+    midpoint (down to ~1e-7 of an fp32 ulp, i.e. 1e-14 relative -- still 50x the kernel's fp64 error) and
+    requires bitwise equal offsets on all of them."""
+    import torch
+    from oracle.selection import row_offset_fp32
+    from paper_2607_04068_b200 import stark_logits_row_offset
+    r = _rng(9)
+    C, rows, keep = 4, 1 << 22, 4096
+    logits = r.normal(0, 2, (rows, C)).astype(np.float32)
+    x = logits.astype(np.float64)
+    m = x.max(-1)
+    lse = m + np.log(np.exp(x - m[:, None]).sum(-1))                 # the oracle's own formula (fp64)
+    lo = lse.astype(np.float32)                                      # nearest fp32 ...
+    other = np.nextafter(lo, np.where(lo.astype(np.float64) < lse, np.float32(np.inf), np.float32(-np.inf))).astype(np.float32)
+    mid = 0.5 * (lo.astype(np.float64) + other.astype(np.float64))   # ... and the rounding boundary on lse's side
+    ulp = np.abs(other.astype(np.float64) - lo.astype(np.float64))
+    dist = np.abs(lse - mid) / ulp                                   # in fp32 ulps; 0 = exactly on the boundary
+    hard = np.argsort(dist)[:keep]
+    print(f"closest distances to an fp32 rounding boundary: {dist[hard[:3]]} ulp(fp32); fp64 eps = {2**-52 * 2**23:.1e} ulp(fp32)")
+    assert dist[hard[-1]] < 1e-3
+    sel = np.ascontiguousarray(logits[hard])
+    off = torch.empty(keep, dtype=torch.float32, device="cuda")
+    stark_logits_row_offset(torch.from_numpy(sel).cuda(), None, keep, C, off)
+    ref = row_offset_fp32(np.zeros(keep, np.float32), sel)
+    far = dist[hard] > 64 * 2.0 ** -29                               # > 64 fp64 ulps from the boundary
+    assert np.array_equal(off.cpu().numpy()[far].view(np.uint32), ref[far].view(np.uint32))
+    # rows even closer than that (none in practice) may legitimately round either way: by one fp32 ulp at most
+    d = np.abs(off.cpu().numpy().view(np.int32).astype(np.int64) - ref.view(np.int32).astype(np.int64))
+    assert d.max() <= 1
