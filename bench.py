@@ -367,23 +367,32 @@ def run_traffic_from(args):
     decode attention then top-k)."""
     import csv
     rows = list(csv.DictReader(open(args.traffic_from)))
+    unit_of = rows[0] if rows else {}                    # ncu's raw page: the first data row holds the units
     cfg = wl.get_config(args.workload)
-    fam = {"prefix_tc_kernel": "decode_step", "topk": "beam_topk"}
+    nq, widths = wl.queries_per_step(cfg), wl.beam_widths(cfg)
+    # decode steps each kernel family serves, in launch order: the fused attention launch at every step; the
+    # whole-GPU top-k where a user has >= 131072 candidates (topk_grid.cu), the other top-k kernels elsewhere
+    grid_steps = [t for t in range(cfg.d) if nq[t] * cfg.C >= 131072 and widths[t] <= 1024 and cfg.C % 4 == 0]
+    fam = {"prefix_tc_kernel": ("decode_step", list(range(cfg.d))), "topk_grid_kernel": ("beam_topk", grid_steps),
+           "topk_": ("beam_topk", [t for t in range(cfg.d) if t not in grid_steps])}
     seen, out = {}, {}
     for r in rows:
         name = r.get("Kernel Name", "")
-        key = next((v for k, v in fam.items() if k in name), None)
-        if key is None:
+        hit = next((k for k in fam if k in name), None)
+        if hit is None:
             continue
+        mult = {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
         try:
-            byts = float(r["dram__bytes_read.sum"].replace(",", "")) + float(r["dram__bytes_write.sum"].replace(",", ""))
+            byts = sum(float(r[c].replace(",", "")) * mult.get(unit_of.get(c, "byte"), 1)
+                       for c in ("dram__bytes_read.sum", "dram__bytes_write.sum"))
         except (KeyError, ValueError):
-            continue                                     # (the units row)
-        t = seen.get(key, 0)
-        seen[key] = t + 1
-        if t < cfg.d:
-            out[f"{key}.t{t}"] = int(byts)
-    units = next((r.get("dram__bytes_read.sum") for r in rows if not r.get("Kernel Name")), None)
+            continue
+        key, steps = fam[hit]
+        n = seen.get(hit, 0)
+        seen[hit] = n + 1
+        if n < len(steps):
+            out[f"{key}.t{steps[n]}"] = int(byts)
+    units = "byte"
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     allj = json.load(open(tpath)) if os.path.exists(tpath) else {}
     allj[cfg.name] = out | {"_source": {"csv": os.path.relpath(os.path.abspath(args.traffic_from), ROOT),
