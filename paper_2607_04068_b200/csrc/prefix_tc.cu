@@ -241,8 +241,10 @@ template <int D> struct TcCfg {
 };
 
 // Suffix-chain scores of one query row (Eq. 14: ancestors and itself), in log2 units of the
-// scaled score, and the element offsets of the chain's rows in the suffix buffers.  Independent of the prefix,
-// so the fused kernel runs it while the first K/V tiles are still in flight.
+// scaled score, and the element offsets of the chain's rows in the suffix buffers.  Independent of the prefix:
+// the fused kernel runs it right after its last softmax iteration, inside the wait for the last MMAs.  (Run
+// ahead of the loop it held the first softmax iteration back: under the kernel's own K/V stream a dependent
+// global load takes 2-3 k cycles, and there are three in a row here.  Measured A/B: 1-2.5 % per launch.)
 template <int D>
 __device__ __forceinline__ void chain_scores(const FusedArgs& fa, float scale_log2, int u, int i, int h, int kv, int n_q,
                                           int Hq, int Hkv, int B, float* y, uint32_t* off_out) {
@@ -699,8 +701,6 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
         // ===================== softmax / correction / epilogue =====================
-        if (FUSED && mine && owner == (int)me && live && fa.level > 0)  // overlaps the first K/V tiles' flight
-            chain_scores<D>(fa, scale_log2, u, i, kv * G + g, kv, n_q, Hq, Hkv, B, ch_y, ch_off);
         if (t == 0 || both) {
             const uint32_t aS = lane_addr + C::COL_S + t * BN;
             const int my_tiles = parity ? (n_tiles - t + 1) / 2 : n_tiles;  // KV tiles of this accumulator set
@@ -796,6 +796,8 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 if (lane == 0) mbar_arrive(bar_pfull + 8 * t);
             }
             // ---- epilogue: O row -> partials ----
+            if (FUSED && mine && owner == (int)me && live && fa.level > 0)  // inside the wait for the last MMAs
+                chain_scores<D>(fa, scale_log2, u, i, kv * G + g, kv, n_q, Hq, Hkv, B, ch_y, ch_off);
             if (FUSED && vpre) {
                 // The V rows of the first two chain levels of this warp's 32 rows go to ring bytes [4, 8) * 32*D*4
                 // (K/V ring tiles 2 and 3; unused by the tail in parity mode without splits) asynchronously, as
