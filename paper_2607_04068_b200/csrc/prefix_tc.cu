@@ -414,6 +414,63 @@ __device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char*
     }
 }
 
+// Tail of the fused kernel for a CTA without splits in pair mode (the large-batch case).  The chain's part of the
+// row -- weights relative to the chain's own maximum m_c, their sum l_c, and vs = sum_t e_t V_t -- is already in
+// registers (chain_partial, run inside the wait for the last MMAs: one global round trip per LEVEL instead of one
+// per level pair and 32-column chunk after it); here it is merged with the prefix part like a second split.
+template <int D>
+__device__ __forceinline__ void fused_finish_single(const FusedArgs& fa, unsigned char* smem_raw, uint32_t ring_off,
+                                                 int blk, int lane, uint32_t aO, bool has, float m_own, float l_own,
+                                                 int u, int n_q, int Hq, int G, int kv, int beam_base, int quarter,
+                                                 float m_c, float l_c, const float (&vs)[D]) {
+    constexpr uint32_t SLOT = 32 * D * 4;
+    constexpr int CPO = D / 8;                          // 16-byte chunks per bf16 row
+    unsigned char* stage = smem_raw + ring_off + (size_t)blk * SLOT;   // bf16 output staging [32][D]
+    const int r = quarter * 32 + lane;
+    const int i = beam_base + r / G;
+    const bool live = i < n_q;
+    tc_fence_after();
+    const float m_p = has ? m_own : -INFINITY;
+    const float m_all = fmaxf(m_p, m_c);
+    const bool any = m_all > -INFINITY;                 // false only for an empty prefix at level 0
+    const float w_p = (any && m_p > -INFINITY) ? fast_exp2(m_p - m_all) : 0.f;
+    const float w_c = (any && m_c > -INFINITY) ? fast_exp2(m_c - m_all) : 0.f;
+    const float denom = fmaf(w_p, l_own, w_c * l_c);
+    const float inv = denom > 0.f ? 1.0f / denom : 0.f;
+    const float wp = w_p * inv, wc = w_c * inv;
+#pragma unroll
+    for (int c = 0; c < D / 32; ++c) {
+        uint32_t o[32];
+        if (has) {
+            tmem_ld32(aO + c * 32, o);
+            tmem_wait_ld();
+        }
+#pragma unroll
+        for (int k4 = 0; k4 < 4; ++k4) {                // 4 chunks of 8 bf16
+            uint32_t pk[4];
+#pragma unroll
+            for (int e2 = 0; e2 < 4; ++e2) {
+                const int x = k4 * 8 + 2 * e2;
+                const float a0 = fmaf(wc, vs[c * 32 + x], has ? wp * __uint_as_float(o[x]) : 0.f);
+                const float a1 = fmaf(wc, vs[c * 32 + x + 1], has ? wp * __uint_as_float(o[x + 1]) : 0.f);
+                const __nv_bfloat162 h = __floats2bfloat162_rn(a0, a1);
+                pk[e2] = *reinterpret_cast<const uint32_t*>(&h);
+            }
+            const int ch = (c * 4 + k4) ^ (lane & (CPO - 1));
+            *reinterpret_cast<uint4*>(stage + (size_t)lane * D * 2 + ch * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        }
+    }
+    __syncwarp();
+    const long long my_row = live ? (long long)(((size_t)u * n_q + i) * Hq + kv * G + r % G) : -1;
+#pragma unroll 4
+    for (int idx = lane; idx < 32 * CPO; idx += 32) {
+        const int l2 = idx / CPO, ch = idx % CPO;
+        const long long row = __shfl_sync(0xffffffffu, my_row, l2);
+        const uint4 v = *reinterpret_cast<const uint4*>(stage + (size_t)l2 * D * 2 + ((ch ^ (l2 & (CPO - 1))) * 16));
+        if (row >= 0) *reinterpret_cast<uint4*>(fa.out + (size_t)row * D + ch * 8) = v;
+    }
+}
+
 // FUSED = false: emit the split-softmax partials (stark_prefix_attn).
 // FUSED = true : the n_splits CTAs of one (Q-tile pair, KV head, user) form a thread-block cluster; they
 //                exchange their partial rows through distributed shared memory, and the owner of each
@@ -701,6 +758,10 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
         // ===================== softmax / correction / epilogue =====================
+        // pair mode without splits: the chain's part of the row stays in registers until the tail (see below)
+        const bool single = FUSED && !parity && n_splits == 1 && mine && fa.level > 0;
+        float m_c = -INFINITY, l_c = 0.f;
+        float vs[FUSED ? D : 1];
         if (t == 0 || both) {
             const uint32_t aS = lane_addr + C::COL_S + t * BN;
             const int my_tiles = parity ? (n_tiles - t + 1) / 2 : n_tiles;  // KV tiles of this accumulator set
@@ -798,6 +859,34 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
             // ---- epilogue: O row -> partials ----
             if (FUSED && mine && owner == (int)me && live && fa.level > 0)  // inside the wait for the last MMAs
                 chain_scores<D>(fa, scale_log2, u, i, kv * G + g, kv, n_q, Hq, Hkv, B, ch_y, ch_off);
+            // pair mode without splits: the chain's weighted V sum, relative to the chain's own maximum, one level
+            // (one global round trip) at a time, also inside that wait
+            if (single) {
+#pragma unroll
+                for (int x = 0; x < D; ++x) vs[x] = 0.f;
+                if (live && fa.level > 0) {
+#pragma unroll 1
+                    for (int t2 = 0; t2 < fa.level; ++t2) m_c = fmaxf(m_c, ch_y[t2]);
+#pragma unroll 1
+                    for (int t2 = 0; t2 < fa.level; ++t2) {
+                        const float e = fast_exp2(ch_y[t2] - m_c);
+                        l_c += e;
+                        const uint4* vp = reinterpret_cast<const uint4*>(((fa.vn && t2 == fa.level - 1) ? fa.vn : fa.vs) + ch_off[t2]);
+                        uint4 vv[D / 8];
+#pragma unroll
+                        for (int c = 0; c < D / 8; ++c) vv[c] = __ldg(vp + c);
+#pragma unroll
+                        for (int c = 0; c < D / 8; ++c) {
+                            const uint32_t va[4] = {vv[c].x, vv[c].y, vv[c].z, vv[c].w};
+#pragma unroll
+                            for (int e2 = 0; e2 < 4; ++e2) {
+                                vs[c * 8 + 2 * e2] = fmaf(e, __uint_as_float(va[e2] << 16), vs[c * 8 + 2 * e2]);
+                                vs[c * 8 + 2 * e2 + 1] = fmaf(e, __uint_as_float(va[e2] & 0xffff0000u), vs[c * 8 + 2 * e2 + 1]);
+                            }
+                        }
+                    }
+                }
+            }
             if (FUSED && vpre) {
                 // The V rows of the first two chain levels of this warp's 32 rows go to ring bytes [4, 8) * 32*D*4
                 // (K/V ring tiles 2 and 3; unused by the tail in parity mode without splits) asynchronously, as
@@ -946,7 +1035,10 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 st_cluster_f2(map_to_rank(ml_base + slot * 256 + (uint32_t)lane * 8, (uint32_t)owner), m_ref, l_sum);
             }
             if (n_splits > 1) cluster_sync_all();                          // B2: all partial rows delivered
-            if (mine && owner == (int)me) {
+            if (single) {
+                fused_finish_single<D>(fa, smem_raw, sKV - smem_u32(smem_raw), blk, lane, aO, n_tiles > 0, m_ref, l_sum,
+                                       u, n_q, Hq, G, kv, (tile0 + t) * beams_per_tile, quarter, m_c, l_c, vs);
+            } else if (mine && owner == (int)me) {
                 if (vpre) { asm volatile("cp.async.wait_group 0;" ::: "memory"); __syncwarp(); }
                 fused_finish<D>(fa, smem_raw, sKV - smem_u32(smem_raw), ob, (int)me, n_splits, lane, aO, n_tiles > 0, m_ref,
                                 l_sum, u, n_q, Hq, G, kv, (tile0 + (parity ? 0 : t)) * beams_per_tile, quarter, ch_y, ch_off,
