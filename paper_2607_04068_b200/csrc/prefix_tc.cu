@@ -476,7 +476,10 @@ __device__ __forceinline__ void fused_finish_single(const FusedArgs& fa, unsigne
 //                exchange their partial rows through distributed shared memory, and the owner of each
 //                32-row block merges them, adds the suffix chain and writes the normalised bf16 output
 //                (stark_decode_attn): no partial ever goes to HBM.
-template <int D, bool FUSED>
+// SINGLE (fused only): pair mode, no splits, level >= 1 -- the instantiation with the register-resident chain part
+//                and fused_finish_single as its tail (its own instantiation: carrying both tails in one kernel cost
+//                the parity-mode and split launches 5-8 %).
+template <int D, bool FUSED, bool SINGLE = false>
 __global__ void __launch_bounds__(kThreadsTC, 1)
 prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                  const __grid_constant__ CUtensorMap tm_v, const int32_t* __restrict__ cu,
@@ -759,9 +762,9 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
         asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
         // ===================== softmax / correction / epilogue =====================
         // pair mode without splits: the chain's part of the row stays in registers until the tail (see below)
-        const bool single = FUSED && !parity && n_splits == 1 && mine && fa.level > 0;
+        const bool single = SINGLE && mine;
         float m_c = -INFINITY, l_c = 0.f;
-        float vs[FUSED ? D : 1];
+        float vs[SINGLE ? D : 1];
         if (t == 0 || both) {
             const uint32_t aS = lane_addr + C::COL_S + t * BN;
             const int my_tiles = parity ? (n_tiles - t + 1) / 2 : n_tiles;  // KV tiles of this accumulator set
@@ -861,7 +864,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 chain_scores<D>(fa, scale_log2, u, i, kv * G + g, kv, n_q, Hq, Hkv, B, ch_y, ch_off);
             // pair mode without splits: the chain's weighted V sum, relative to the chain's own maximum, one level
             // (one global round trip) at a time, also inside that wait
-            if (single) {
+            if constexpr (SINGLE) if (single) {
 #pragma unroll
                 for (int x = 0; x < D; ++x) vs[x] = 0.f;
                 if (live && fa.level > 0) {
@@ -1035,9 +1038,10 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 st_cluster_f2(map_to_rank(ml_base + slot * 256 + (uint32_t)lane * 8, (uint32_t)owner), m_ref, l_sum);
             }
             if (n_splits > 1) cluster_sync_all();                          // B2: all partial rows delivered
-            if (single) {
-                fused_finish_single<D>(fa, smem_raw, sKV - smem_u32(smem_raw), blk, lane, aO, n_tiles > 0, m_ref, l_sum,
-                                       u, n_q, Hq, G, kv, (tile0 + t) * beams_per_tile, quarter, m_c, l_c, vs);
+            if constexpr (SINGLE) {
+                if (single)
+                    fused_finish_single<D>(fa, smem_raw, sKV - smem_u32(smem_raw), blk, lane, aO, n_tiles > 0, m_ref,
+                                           l_sum, u, n_q, Hq, G, kv, (tile0 + t) * beams_per_tile, quarter, m_c, l_c, vs);
             } else if (mine && owner == (int)me) {
                 if (vpre) { asm volatile("cp.async.wait_group 0;" ::: "memory"); __syncwarp(); }
                 fused_finish<D>(fa, smem_raw, sKV - smem_u32(smem_raw), ob, (int)me, n_splits, lane, aO, n_tiles > 0, m_ref,
@@ -1114,11 +1118,14 @@ int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, 
     if (!attr_done.here()) {
         STARK_CUDA_TRY(cudaFuncSetAttribute(prefix_tc_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             TcCfg<D>::SMEM_BYTES));
+        STARK_CUDA_TRY(cudaFuncSetAttribute(prefix_tc_kernel<D, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            TcCfg<D>::SMEM_BYTES));
         attr_done.here() = true;
     }
     const int M = n_q * p.G;
     const int parity = prefix_tc_parity(p, n_q, n_splits) ? 1 : 0;
     const int rows_per_cta = parity ? BM : 2 * BM;
+    const bool single = !parity && n_splits == 1 && fa.level > 0;   // see the kernel's template parameters
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((M + rows_per_cta - 1) / rows_per_cta, p.Hkv * n_splits, p.B);
     cfg.blockDim = dim3(kThreadsTC);
@@ -1128,9 +1135,9 @@ int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, 
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = n_splits; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = n_splits > 1 ? 1 : 0;   // a single split needs no cluster launch
-    STARK_CUDA_TRY(cudaLaunchKernelEx(&cfg, prefix_tc_kernel<D, true>, tq, tk, tv, cu, (float*)nullptr,
-                                      (float*)nullptr, (float*)nullptr, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits,
-                                      p.scale * kLog2e, parity, lpt, fa));
+    STARK_CUDA_TRY(cudaLaunchKernelEx(&cfg, single ? prefix_tc_kernel<D, true, true> : prefix_tc_kernel<D, true, false>,
+                                      tq, tk, tv, cu, (float*)nullptr, (float*)nullptr, (float*)nullptr, p.B, n_q,
+                                      p.Hq, p.Hkv, p.G, n_splits, p.scale * kLog2e, parity, lpt, fa));
     return STARK_OK;
 }
 
