@@ -246,13 +246,16 @@ template <int D> struct TcCfg {
 // ahead of the loop it held the first softmax iteration back: under the kernel's own K/V stream a dependent
 // global load takes 2-3 k cycles, and there are three in a row here.  Measured A/B: 1-2.5 % per launch.)
 template <int D>
-__device__ __forceinline__ void chain_scores(const FusedArgs& fa, float scale_log2, int u, int i, int h, int kv, int n_q,
-                                          int Hq, int Hkv, int B, float* y, uint32_t* off_out) {
+__device__ __forceinline__ void chain_scores(const FusedArgs& fa, float scale_log2, int u, int i, int kv, int n_q,
+                                          int Hkv, int B, const unsigned char* q_tile, int r, float* y,
+                                          uint32_t* off_out) {
     const size_t level_stride = (size_t)B * fa.Wmax * Hkv * D;
+    // the query row comes from the Q tile TMA left in shared memory (128-byte swizzle: 16-byte chunk c of row r of a
+    // 64-column box sits at chunk c ^ (r & 7)); conflict-free, and a quarter of this function's global traffic less
     uint4 qv[D / 8];
-    const uint4* qp = reinterpret_cast<const uint4*>(fa.q + (((size_t)u * n_q + i) * Hq + h) * D);
 #pragma unroll
-    for (int c = 0; c < D / 8; ++c) qv[c] = __ldg(qp + c);
+    for (int c = 0; c < D / 8; ++c)
+        qv[c] = *reinterpret_cast<const uint4*>(q_tile + (c / 8) * (BM * 128) + r * 128 + (((c % 8) ^ (r & 7)) << 4));
     const bool inl = fa.kn != nullptr;
     int chain_of = i;                                   // whose row of `anc` holds this query's ancestors
     if (inl && fa.level >= 2) chain_of = min(max(__ldg(fa.parent + (size_t)u * n_q + i), 0), fa.Wmax - 1);
@@ -598,7 +601,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
         fence_barrier_init();
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         const int beam0 = u * n_q + tile0 * beams_per_tile;
-        if (n_tiles > 0) {                               // (a fused CTA with an empty split loads nothing)
+        if (n_tiles > 0 || (FUSED && fa.level > 0)) {    // (an empty split still needs q for the chain scores)
             mbar_expect_tx(bar_q, (two ? 2 : 1) * C::TILE_BYTES);
             for (int t = 0; t < (two ? 2 : 1); ++t)
 #pragma unroll
@@ -860,8 +863,10 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
                 if (lane == 0) mbar_arrive(bar_pfull + 8 * t);
             }
             // ---- epilogue: O row -> partials ----
+            if (FUSED && fa.level > 0 && n_tiles == 0) mbar_wait(bar_q, 0);   // (otherwise S was ready: so was Q)
             if (FUSED && mine && owner == (int)me && live && fa.level > 0)  // inside the wait for the last MMAs
-                chain_scores<D>(fa, scale_log2, u, i, kv * G + g, kv, n_q, Hq, Hkv, B, ch_y, ch_off);
+                chain_scores<D>(fa, scale_log2, u, i, kv, n_q, Hkv, B,
+                                smem_raw + (sQ - smem_u32(smem_raw)) + (parity ? 0 : t) * C::TILE_BYTES, r, ch_y, ch_off);
             // pair mode without splits: the chain's weighted V sum, relative to the chain's own maximum, one level
             // (one global round trip) at a time, also inside that wait
             if constexpr (SINGLE) if (single) {
