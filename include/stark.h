@@ -261,6 +261,35 @@ int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_
                     void* ws, size_t ws_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------
+ * A3 without a caller workspace: stark_beam_topk_static
+ *
+ * stark_beam_topk (same definition: Eq. 1, 257, 263, 306; same
+ * kernels, same arguments, bit-identical result) for callers that cannot
+ * allocate device memory: code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc.  The workspace is a static device array
+ * inside the library:
+ *   - it takes STARK_TOPK_STATIC_SCRATCH_BYTES of device memory on every GPU
+ *     that loads the library, until the process exits;
+ *   - a problem whose stark_workspace_bytes(STARK_CALL_BEAM_TOPK, ...) exceeds
+ *     it is rejected with STARK_ERR_WORKSPACE (nothing is launched); on B200
+ *     that is B > 29 users with W_in*C >= 131072 -- use stark_beam_topk then;
+ *   - the call allocates nothing (no cudaMalloc / cudaFree / allocating
+ *     library routine): argument checks, one cudaMemsetAsync that clears the
+ *     part of the array this call uses, the kernel launches, all on `stream`;
+ *   - ALL CALLS ON ONE GPU SHARE THE ARRAY: calls that may overlap on the GPU
+ *     (streams without an ordering between them, several host threads) race
+ *     and give undefined results.  Order them, or use stark_beam_topk with a
+ *     workspace each.
+ * logp, score_or_null, out_*: device pointers, as for stark_beam_topk.
+ * Errors: INVALID_ARG as stark_beam_topk, WORKSPACE (beyond the static
+ * maximum), UNSUPPORTED (not an sm_100 device), CUDA.
+ */
+#define STARK_TOPK_STATIC_SCRATCH_BYTES (9u << 20)
+int stark_beam_topk_static(const float* logp, const float* score_or_null, int B, int W_in, int C,
+                           int W_out, float* out_score, int32_t* out_parent, int32_t* out_code,
+                           void* stream);
+
+/* ---------------------------------------------------------------------------
  * A3'. Beam selection straight from raw logits  (
  *      DESIGN.md reading R22)
  *

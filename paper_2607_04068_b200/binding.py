@@ -20,7 +20,7 @@ STARK_F32, STARK_BF16 = 0, 1
 CALL_PREFIX_ATTN, CALL_TREE_ATTN_STEP, CALL_BEAM_TOPK, CALL_KV_APPEND_REORG, CALL_BEAM_TOPK_LOGITS = 0, 1, 2, 3, 4
 EXPORTS = (
     "stark_prefix_attn", "stark_prefix_attn_plan", "stark_tree_attn_step", "stark_decode_attn", "stark_decode_step",
-    "stark_beam_topk", "stark_logits_row_offset", "stark_beam_topk_logits",
+    "stark_beam_topk", "stark_beam_topk_static", "stark_logits_row_offset", "stark_beam_topk_logits",
     "stark_kv_append_reorg", "stark_workspace_bytes", "stark_suffix_bytes",
     "stark_anc_bytes", "stark_version", "stark_status_string", "stark_last_cuda_error",
 )
@@ -71,6 +71,9 @@ def lib() -> ctypes.CDLL:
     L.stark_beam_topk.restype = c_int
     L.stark_beam_topk.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p,
                                   c_void_p, c_size_t, c_void_p]
+    L.stark_beam_topk_static.restype = c_int
+    L.stark_beam_topk_static.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p,
+                                         c_void_p]
     L.stark_logits_row_offset.restype = c_int
     L.stark_logits_row_offset.argtypes = [c_void_p, c_void_p, c_int64, c_int, c_void_p, c_void_p]
     L.stark_beam_topk_logits.restype = c_int
@@ -175,6 +178,23 @@ def stark_beam_topk(logp: torch.Tensor, score: Optional[torch.Tensor], B: int, W
     _check(lib().stark_beam_topk(_ptr(logp), _ptr(score), B, W_in, C, W_out, _ptr(out_score), _ptr(out_parent),
                                  _ptr(out_code), _ptr(ws), ws.numel() * ws.element_size() if ws is not None else 0,
                                  _stream()), "stark_beam_topk")
+
+
+#: size of the library's static top-k scratch array (include/stark.h: STARK_TOPK_STATIC_SCRATCH_BYTES)
+TOPK_STATIC_SCRATCH_BYTES = 9 << 20
+
+
+def stark_beam_topk_static(logp: torch.Tensor, score: Optional[torch.Tensor], B: int, W_in: int, C: int, W_out: int,
+                           out_score: torch.Tensor, out_parent: torch.Tensor, out_code: torch.Tensor) -> None:
+    """stark_beam_topk on the library's own static scratch array: allocates nothing, not safe for calls that
+    overlap on the GPU, limited to problems whose workspace fits TOPK_STATIC_SCRATCH_BYTES."""
+    rc = lib().stark_beam_topk_static(_ptr(logp), _ptr(score), B, W_in, C, W_out, _ptr(out_score), _ptr(out_parent),
+                                      _ptr(out_code), _stream())
+    if rc == -3:
+        need = stark_workspace_bytes(make_shape(B, 1, 1, 64, 1, max(W_in, 1), torch.float32), CALL_BEAM_TOPK, W_in, C)
+        raise StarkError(rc, f"stark_beam_topk_static (B={B}, W_in={W_in}, C={C} needs {need} bytes of scratch, the "
+                             f"static array holds {TOPK_STATIC_SCRATCH_BYTES}: use stark_beam_topk with a workspace)")
+    _check(rc, "stark_beam_topk_static")
 
 
 def stark_logits_row_offset(logits: torch.Tensor, score: Optional[torch.Tensor], rows: int, C: int,

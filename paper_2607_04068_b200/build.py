@@ -22,7 +22,7 @@ OBJ_DIR = os.path.join(HERE, "build")
 CALIB_DIR = os.path.join(HERE, "calib")
 CALIB_LIB = os.path.join(CALIB_DIR, "libstark_calib.so")
 
-SOURCES = ["api.cu", "append.cu", "tree_attn.cu", "prefix_simt.cu", "prefix_tc.cu", "topk.cu", "topk_grid.cu", "logits_offset.cu"]
+SOURCES = ["api.cu", "append.cu", "tree_attn.cu", "prefix_simt.cu", "prefix_tc.cu", "topk.cu", "topk_grid.cu", "topk_static.cu", "logits_offset.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC]
 

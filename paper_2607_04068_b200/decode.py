@@ -124,6 +124,15 @@ def beam_topk(logp: torch.Tensor, score: Optional[torch.Tensor], W_out: int,
     return out
 
 
+def beam_topk_static(logp: torch.Tensor, score: Optional[torch.Tensor], W_out: int,
+                     out: Tuple[torch.Tensor, torch.Tensor, torch.Tensor]):
+    """beam_topk for callers that must not allocate: the outputs are the caller's, the scratch memory is the
+    library's static array (include/stark.h: stark_beam_topk_static -- its size limit and the no-overlap rule)."""
+    B, W_in, C = logp.shape
+    sb.stark_beam_topk_static(logp, score, B, W_in, C, W_out, out[0], out[1], out[2])
+    return out
+
+
 def beam_topk_logits(logits: torch.Tensor, score: Optional[torch.Tensor], W_out: int,
                      out: Optional[Tuple[torch.Tensor, torch.Tensor, torch.Tensor]] = None,
                      ws: Optional[torch.Tensor] = None):
