@@ -102,6 +102,32 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm,
         ::"r"(dst), "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 
+// Store one box of a 4-d tensor map from shared memory (bulk async group of the issuing thread); elements outside
+// the tensor are not written.
+__device__ __forceinline__ void tma_store_4d(const CUtensorMap* tm, uint32_t src, int c0, int c1, int c2, int c3) {
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5}], [%1];"
+                 ::"l"(tm), "r"(src), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+
+// The 32 finished bf16 rows of one warp, staged at `stage` (1024-byte aligned) in the layout of a 128-byte-swizzled
+// TMA box per 64 columns ([D / 64][32 rows][128 B], 16-byte chunk c of row r at c ^ (r & 7)), go to
+// out[u, beam, head, :] with one TMA store per box.  Row r of the warp is (beam, head) = (beam0 + r / hb, head0 +
+// r % hb) with hb = min(G, 32) heads per beam in the box; beams >= n_q lie outside the tensor map and are clipped.
+// (The copy loop this replaces took 2.2-2.7 k cycles per warp: 16 rounds of shared-memory load, shuffle, store.)
+template <int D>
+__device__ __forceinline__ void store_rows_tma(const CUtensorMap* tm_o, const unsigned char* stage, int lane, int u,
+                                            int head0, int beam0) {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // this thread's staged row -> async proxy
+    __syncwarp();
+    if (lane == 0) {
+#pragma unroll
+        for (int bx = 0; bx < D / 64; ++bx)
+            tma_store_4d(tm_o, smem_u32(stage) + bx * (32 * 128), bx * 64, head0, beam0, u);
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the staging memory may go (CTA exit)
+    }
+}
+
 __device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -299,10 +325,10 @@ template <int D>
 __device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char* smem_raw, uint32_t ring_off, int ob, int me,
                                           int ns, int lane, uint32_t aO, bool has, float m_own, float l_own,
                                           int u, int n_q, int Hq, int G, int kv, int beam_base, int quarter,
-                                          float* ch_y, const uint32_t* ch_off, const unsigned char* vstage) {
+                                          float* ch_y, const uint32_t* ch_off, const unsigned char* vstage,
+                                          const CUtensorMap* tm_o) {
     constexpr uint32_t SLOT = 32 * D * 4;
     constexpr int CPR = D / 4;                          // 16-byte chunks per fp32 row
-    constexpr int CPO = D / 8;                          // 16-byte chunks per bf16 row
     unsigned char* ring = smem_raw + ring_off;
     // this block's own slot is never written remotely: bf16 output staging [32][D] + per-lane scratch
     unsigned char* stage = ring + (size_t)(ob * ns + me) * SLOT;
@@ -401,20 +427,12 @@ __device__ __forceinline__ void fused_finish(const FusedArgs& fa, unsigned char*
                 const __nv_bfloat162 h = __floats2bfloat162_rn(acc[k4 * 8 + 2 * e2] * inv, acc[k4 * 8 + 2 * e2 + 1] * inv);
                 pk[e2] = *reinterpret_cast<const uint32_t*>(&h);
             }
-            const int ch = (c * 4 + k4) ^ (lane & (CPO - 1));
-            *reinterpret_cast<uint4*>(stage + (size_t)lane * D * 2 + ch * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+            const int ch = c * 4 + k4;                  // 16-byte chunk of the row: box ch / 8, swizzled inside it
+            *reinterpret_cast<uint4*>(stage + (ch >> 3) * (32 * 128) + lane * 128 + (((ch & 7) ^ (lane & 7)) << 4)) =
+                make_uint4(pk[0], pk[1], pk[2], pk[3]);
         }
     }
-    __syncwarp();
-    // lane l knows where row l goes (-1: dead row); the copy loop fetches that by shuffle
-    const long long my_row = live ? (long long)(((size_t)u * n_q + i) * Hq + kv * G + r % G) : -1;
-#pragma unroll 4
-    for (int idx = lane; idx < 32 * CPO; idx += 32) {
-        const int l2 = idx / CPO, ch = idx % CPO;
-        const long long row = __shfl_sync(0xffffffffu, my_row, l2);
-        const uint4 v = *reinterpret_cast<const uint4*>(stage + (size_t)l2 * D * 2 + ((ch ^ (l2 & (CPO - 1))) * 16));
-        if (row >= 0) *reinterpret_cast<uint4*>(fa.out + (size_t)row * D + ch * 8) = v;
-    }
+    store_rows_tma<D>(tm_o, stage, lane, u, kv * G + (quarter * 32) % G, beam_base + (quarter * 32) / G);
 }
 
 // Tail of the fused kernel for a CTA without splits in pair mode (the large-batch case).  The chain's part of the
@@ -425,13 +443,9 @@ template <int D>
 __device__ __forceinline__ void fused_finish_single(const FusedArgs& fa, unsigned char* smem_raw, uint32_t ring_off,
                                                  int blk, int lane, uint32_t aO, bool has, float m_own, float l_own,
                                                  int u, int n_q, int Hq, int G, int kv, int beam_base, int quarter,
-                                                 float m_c, float l_c, const float (&vs)[D]) {
+                                                 float m_c, float l_c, const float (&vs)[D], const CUtensorMap* tm_o) {
     constexpr uint32_t SLOT = 32 * D * 4;
-    constexpr int CPO = D / 8;                          // 16-byte chunks per bf16 row
-    unsigned char* stage = smem_raw + ring_off + (size_t)blk * SLOT;   // bf16 output staging [32][D]
-    const int r = quarter * 32 + lane;
-    const int i = beam_base + r / G;
-    const bool live = i < n_q;
+    unsigned char* stage = smem_raw + ring_off + (size_t)blk * SLOT;   // bf16 output staging (store_rows_tma)
     tc_fence_after();
     const float m_p = has ? m_own : -INFINITY;
     const float m_all = fmaxf(m_p, m_c);
@@ -459,19 +473,12 @@ __device__ __forceinline__ void fused_finish_single(const FusedArgs& fa, unsigne
                 const __nv_bfloat162 h = __floats2bfloat162_rn(a0, a1);
                 pk[e2] = *reinterpret_cast<const uint32_t*>(&h);
             }
-            const int ch = (c * 4 + k4) ^ (lane & (CPO - 1));
-            *reinterpret_cast<uint4*>(stage + (size_t)lane * D * 2 + ch * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+            const int ch = c * 4 + k4;                  // 16-byte chunk of the row: box ch / 8, swizzled inside it
+            *reinterpret_cast<uint4*>(stage + (ch >> 3) * (32 * 128) + lane * 128 + (((ch & 7) ^ (lane & 7)) << 4)) =
+                make_uint4(pk[0], pk[1], pk[2], pk[3]);
         }
     }
-    __syncwarp();
-    const long long my_row = live ? (long long)(((size_t)u * n_q + i) * Hq + kv * G + r % G) : -1;
-#pragma unroll 4
-    for (int idx = lane; idx < 32 * CPO; idx += 32) {
-        const int l2 = idx / CPO, ch = idx % CPO;
-        const long long row = __shfl_sync(0xffffffffu, my_row, l2);
-        const uint4 v = *reinterpret_cast<const uint4*>(stage + (size_t)l2 * D * 2 + ((ch ^ (l2 & (CPO - 1))) * 16));
-        if (row >= 0) *reinterpret_cast<uint4*>(fa.out + (size_t)row * D + ch * 8) = v;
-    }
+    store_rows_tma<D>(tm_o, stage, lane, u, kv * G + (quarter * 32) % G, beam_base + (quarter * 32) / G);
 }
 
 // FUSED = false: emit the split-softmax partials (stark_prefix_attn).
@@ -485,7 +492,8 @@ __device__ __forceinline__ void fused_finish_single(const FusedArgs& fa, unsigne
 template <int D, bool FUSED, bool SINGLE = false>
 __global__ void __launch_bounds__(kThreadsTC, 1)
 prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
-                 const __grid_constant__ CUtensorMap tm_v, const int32_t* __restrict__ cu,
+                 const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_o,
+                 const int32_t* __restrict__ cu,
                  float* __restrict__ pm, float* __restrict__ pl, float* __restrict__ po, int B, int n_q,
                  int Hq, int Hkv, int G, int n_splits, float scale_log2, int parity, int lpt, const FusedArgs fa) {
     // Two TMEM accumulator sets (S_t/P_t, O_t), t = 0, 1, each served by its own softmax warpgroup:
@@ -594,6 +602,7 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_k) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_v) : "memory");
+        if (FUSED) asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_o) : "memory");
         mbar_init(bar_q, 1);
         for (int s = 0; s < NS; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
         for (int t = 0; t < 2; ++t) { mbar_init(bar_sfull + 8 * t, 1); mbar_init(bar_pfull + 8 * t, kSoftmaxThreads / 32); }
@@ -1046,12 +1055,14 @@ prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant
             if constexpr (SINGLE) {
                 if (single)
                     fused_finish_single<D>(fa, smem_raw, sKV - smem_u32(smem_raw), blk, lane, aO, n_tiles > 0, m_ref,
-                                           l_sum, u, n_q, Hq, G, kv, (tile0 + t) * beams_per_tile, quarter, m_c, l_c, vs);
+                                           l_sum, u, n_q, Hq, G, kv, (tile0 + t) * beams_per_tile, quarter, m_c, l_c, vs,
+                                           &tm_o);
             } else if (mine && owner == (int)me) {
                 if (vpre) { asm volatile("cp.async.wait_group 0;" ::: "memory"); __syncwarp(); }
                 fused_finish<D>(fa, smem_raw, sKV - smem_u32(smem_raw), ob, (int)me, n_splits, lane, aO, n_tiles > 0, m_ref,
                                 l_sum, u, n_q, Hq, G, kv, (tile0 + (parity ? 0 : t)) * beams_per_tile, quarter, ch_y, ch_off,
-                                vpre ? smem_raw + (sKV - smem_u32(smem_raw)) + (size_t)(4 + quarter) * (32 * D * 4) : nullptr);
+                                vpre ? smem_raw + (sKV - smem_u32(smem_raw)) + (size_t)(4 + quarter) * (32 * D * 4) : nullptr,
+                                &tm_o);
             }
             tc_fence_before();
         }
@@ -1096,6 +1107,21 @@ bool make_map(CUtensorMap* tm, const void* base, int D, int n1, long long n2, in
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// bf16 tensor out[B][n_q][Hq][D] as a 4-d map; box = 64 columns x hb heads x bb beams x 1 user (the 32 rows a warp
+// finishes), 128-byte swizzle
+bool make_map_out(CUtensorMap* tm, const void* base, int D, int Hq, int n_q, int B, int G) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return false;
+    const int hb = G < 32 ? G : 32, bb = 32 / hb;
+    cuuint64_t dims[4] = {(cuuint64_t)D, (cuuint64_t)Hq, (cuuint64_t)n_q, (cuuint64_t)B};
+    cuuint64_t strides[3] = {(cuuint64_t)D * 2, (cuuint64_t)Hq * D * 2, (cuuint64_t)n_q * Hq * D * 2};
+    cuuint32_t box[4] = {64, (cuuint32_t)hb, (cuuint32_t)bb, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <int D>
 int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, int n_q,
              const int32_t* cu, int n_splits, int lpt, float* pm, float* pl, float* po, cudaStream_t st) {
@@ -1110,15 +1136,16 @@ int launch_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const 
     const int rows_per_cta = parity ? BM : 2 * BM;                  // one Q tile, or a pair of them
     dim3 grid((M + rows_per_cta - 1) / rows_per_cta, p.Hkv * n_splits, p.B);
     prefix_tc_kernel<D, false><<<grid, kThreadsTC, TcCfg<D>::SMEM_BYTES, st>>>(
-        tq, tk, tv, cu, pm, pl, po, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits, p.scale * kLog2e, parity, lpt, FusedArgs{});
+        tq, tk, tv, tq /*unused*/, cu, pm, pl, po, p.B, n_q, p.Hq, p.Hkv, p.G, n_splits, p.scale * kLog2e, parity, lpt,
+        FusedArgs{});
     STARK_LAUNCH_CHECK();
     return STARK_OK;
 }
 
 // fused launch: the n_splits CTAs of one (pair, KV head, user) are a cluster along y
 template <int D>
-int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, int n_q,
-                   const int32_t* cu, int n_splits, int lpt, const FusedArgs& fa, cudaStream_t st) {
+int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
+                   const CUtensorMap& to, int n_q, const int32_t* cu, int n_splits, int lpt, const FusedArgs& fa, cudaStream_t st) {
     static PerDevice<bool> attr_done;
     if (!attr_done.here()) {
         STARK_CUDA_TRY(cudaFuncSetAttribute(prefix_tc_kernel<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -1141,7 +1168,7 @@ int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, 
     at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = n_splits; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = n_splits > 1 ? 1 : 0;   // a single split needs no cluster launch
     STARK_CUDA_TRY(cudaLaunchKernelEx(&cfg, single ? prefix_tc_kernel<D, true, true> : prefix_tc_kernel<D, true, false>,
-                                      tq, tk, tv, cu, (float*)nullptr, (float*)nullptr, (float*)nullptr, p.B, n_q,
+                                      tq, tk, tv, to, cu, (float*)nullptr, (float*)nullptr, (float*)nullptr, p.B, n_q,
                                       p.Hq, p.Hkv, p.G, n_splits, p.scale * kLog2e, parity, lpt, fa));
     return STARK_OK;
 }
@@ -1188,9 +1215,10 @@ int launch_decode_fused(const Dims& p, const void* q, int n_q, int level, const 
                         const int32_t* cu, int total_tokens, int max_len, int n_splits, const void* ks, const void* vs,
                         const int32_t* anc_level, void* out, cudaStream_t st, const void* kn, const void* vn,
                         const int32_t* parent, int32_t* anc_new) {
-    CUtensorMap tq, tk, tv;
+    CUtensorMap tq, tk, tv, to;
     if (!make_map(&tq, q, p.D, p.Hq, (long long)p.B * n_q, p.G, BM / p.G) ||
-        !make_map(&tk, k, p.D, p.Hkv, total_tokens, 1, BN) || !make_map(&tv, v, p.D, p.Hkv, total_tokens, 1, BN)) {
+        !make_map(&tk, k, p.D, p.Hkv, total_tokens, 1, BN) || !make_map(&tv, v, p.D, p.Hkv, total_tokens, 1, BN) ||
+        !make_map_out(&to, out, p.D, p.Hq, n_q, p.B, p.G)) {
         last_cuda_error_ref() = (int)cudaErrorInvalidValue;
         return STARK_ERR_CUDA;
     }
@@ -1200,8 +1228,8 @@ int launch_decode_fused(const Dims& p, const void* q, int n_q, int level, const 
     fa.level = level; fa.Wmax = p.Wmax; fa.d = p.d; fa.scale = p.scale;
     fa.kn = (const __nv_bfloat16*)kn; fa.vn = (const __nv_bfloat16*)vn; fa.parent = parent; fa.anc_new = anc_new;
     const int lpt = ragged_batch(p, total_tokens, max_len);
-    if (p.D == 128) return launch_fused_d<128>(p, tq, tk, tv, n_q, cu, n_splits, lpt, fa, st);
-    return launch_fused_d<64>(p, tq, tk, tv, n_q, cu, n_splits, lpt, fa, st);
+    if (p.D == 128) return launch_fused_d<128>(p, tq, tk, tv, to, n_q, cu, n_splits, lpt, fa, st);
+    return launch_fused_d<64>(p, tq, tk, tv, to, n_q, cu, n_splits, lpt, fa, st);
 }
 
 }  // namespace stark
