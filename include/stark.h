@@ -51,6 +51,10 @@
  *   part_m, part_l  [n_splits, B, n_q, Hq] fp32
  *   part_o          [n_splits, B, n_q, Hq, D] fp32
  *   logp            [B, W_in, C] fp32;  score [B, W_in] fp32
+ * Alignment: every tensor pointer is 16-byte aligned (bf16 q / k_prefix /
+ * v_prefix / out are read and written through TMA tensor maps and 16-byte
+ * vectors; a misaligned bf16 pointer makes the call return STARK_ERR_CUDA with
+ * cudaErrorInvalidValue, nothing is launched).
  */
 #ifndef STARK_H_
 #define STARK_H_
