@@ -126,6 +126,10 @@ size_t topk_grid_workspace_bytes(int B, int W_in, int C);
 int launch_topk_grid(const float* logp, const float* score, int B, int W_in, int C, int W_out,
                      float* out_score, int32_t* out_parent, int32_t* out_code, void* ws, size_t ws_bytes,
                      cudaStream_t st);
+// topk_grid.cu: wide selections (W_out <= 1024) over small candidate sets (N <= 8192): R independent CTAs per user
+bool topk_wide_serves(long long N, int W_out);
+int launch_topk_wide(const float* logp, const float* score, int B, int W_in, int C, int W_out,
+                     float* out_score, int32_t* out_parent, int32_t* out_code, cudaStream_t st);
 int launch_row_offset(const float* logits, const float* score, long long rows, int C, float* offset,
                       cudaStream_t st);
 

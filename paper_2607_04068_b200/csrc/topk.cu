@@ -9,8 +9,11 @@
 // Three kernels by problem size (launch_topk): N <= 512 candidates per user: one
 // 256-thread CTA ranking by counting (topk_small_kernel); N <= 16384 and
 // W_out <= 256: one 1024-thread CTA per user, bound from per-thread maxima +
-// ranking by counting (topk_mid_kernel); otherwise the cluster kernel described
-// here (topk_kernel).  All three produce the same total order.
+// ranking by counting (topk_mid_kernel); N <= 8192, W_out <= 1024 and B <= 16
+// (decode step 0 with a wide beam): R independent CTAs per user, bound by
+// bisection, every CTA ranks a share (topk_wide_kernel in topk_grid.cu); from
+// 131 072 candidates per user the whole-GPU kernel of topk_grid.cu; otherwise
+// the cluster kernel described here (topk_kernel).  All produce the same order.
 // stark_beam_topk_logits (reading R22) feeds the same kernels (raw logits, per-beam offset from
 // logits_offset.cu); for a single-row user the small kernel computes that offset itself (kFold).
 //
@@ -1032,6 +1035,11 @@ int launch_topk(const float* logp, const float* score, int B, int W_in, int C, i
                                                                                  out_score, out_parent, out_code);
         STARK_LAUNCH_CHECK();
         return STARK_OK;
+    }
+    // wide selections over small candidate sets (decode step 0 with a wide beam): independent CTAs, no cluster
+    if (topk_wide_serves(N, W_out)) {
+        const int rc = launch_topk_wide(logp, score, B, W_in, C, W_out, out_score, out_parent, out_code, st);
+        if (rc != STARK_ERR_UNSUPPORTED) return rc;
     }
     // large candidate sets: the whole GPU on every user (topk_grid.cu); UNSUPPORTED = shape not served there
     if (ws) {

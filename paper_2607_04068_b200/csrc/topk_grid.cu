@@ -799,6 +799,142 @@ topk_grid_kernel(const float* __restrict__ logp, const float* __restrict__ score
     PROF(8);
 }
 
+// ---- wide selections over SMALL candidate sets (decode step 0 with a wide beam) ---------------------------------
+// N <= 8192 candidates per user, W_out up to 1024 (512 of the 8192 first-level codes; config 4: 512
+// of 1024).  The cluster kernel of topk.cu spends 14.5 us there, nearly all of it latency: cluster launch, radix
+// passes with cluster barriers, a one-CTA sort.  Here R CTAs per user work WITHOUT talking to each other: each of
+// them reads all N keys (32 KB, the second reader finds them in L2), finds by bisection on the order-preserving
+// uint32 image of the key -- warp votes, a block barrier per step -- a bound with at most K + K/32 keys at or
+// above it (exact ties at the K-th key: a second bisection on the index inside the tie), gathers those survivors
+// as composites (~ord . index) in shared memory, and ranks ITS share of them (by a hash of the index) by counting.
+// All CTAs of a user hold the same survivor set (the counts are exact), so the ranks agree without any exchange;
+// rank r writes row r.
+constexpr int kWideNV = 16;                       // keys per thread
+constexpr int kWideMaxN = kThreads * kWideNV;     // 8192
+constexpr int kWideCap = 2048;                    // survivors (>= kWideMaxK + kWideMaxK / 32)
+constexpr int kWideMaxK = 1024;
+
+__global__ void __launch_bounds__(kThreads, 2)
+topk_wide_kernel(const float* __restrict__ logp, const float* __restrict__ score, int W_in, int C, int c_shift,
+                 int W_out, float* __restrict__ out_score, int32_t* __restrict__ out_parent,
+                 int32_t* __restrict__ out_code, int R) {
+    __shared__ Shared sh;
+    __shared__ unsigned long long ent[kWideCap];
+    const int s = blockIdx.x, u = blockIdx.y;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    Keys ks;
+    ks.N = (uint32_t)((long long)W_in * C);
+    ks.lp = logp + (size_t)u * ks.N;
+    ks.sc = score ? score + (size_t)u * W_in : nullptr;
+    ks.C = C; ks.c_shift = c_shift;
+    const uint32_t N = ks.N, K = (uint32_t)W_out;
+    if (tid == 0) sh.cursor = 0;
+
+    // ---- all keys of the user, as ord (0 = no key), in registers: key x of this thread has index x * 512 + tid ----
+    uint32_t v[kWideNV];
+    {
+        float lv[kWideNV];
+#pragma unroll
+        for (int x = 0; x < kWideNV; ++x) {
+            const uint32_t idx = (uint32_t)(x * kThreads + tid);
+            lv[x] = __ldg(ks.lp + min(idx, N - 1));
+        }
+#pragma unroll
+        for (int x = 0; x < kWideNV; ++x) {
+            const uint32_t idx = (uint32_t)(x * kThreads + tid);
+            v[x] = idx < N ? ord_of(__fadd_rn(ks.score_of(ks.row_of(idx)), lv[x])) : 0u;
+        }
+    }
+    // block-wide number of keys for which `pred(x)` holds (block-uniform; two barriers)
+    auto block_count = [&](auto pred) -> uint32_t {
+        uint32_t c = 0;
+#pragma unroll
+        for (int x = 0; x < kWideNV; ++x) c += __popc(__ballot_sync(0xffffffffu, pred(x)));
+        if (lane == 0) sh.wcnt[warp] = c;
+        __syncthreads();
+        c = __reduce_add_sync(0xffffffffu, lane < kWarps ? sh.wcnt[lane] : 0u);
+        __syncthreads();
+        return c;
+    };
+    // ---- range of the keys -----------------------------------------------------------------------------------------
+    uint32_t vmax = 0u, vmin = 0xffffffffu;
+#pragma unroll
+    for (int x = 0; x < kWideNV; ++x)
+        if (v[x]) { vmax = max(vmax, v[x]); vmin = min(vmin, v[x]); }
+    vmax = __reduce_max_sync(0xffffffffu, vmax);
+    vmin = __reduce_min_sync(0xffffffffu, vmin);
+    if (lane == 0) { sh.wmax[warp] = vmax; sh.wmin[warp] = vmin; }
+    __syncthreads();
+    vmax = __reduce_max_sync(0xffffffffu, lane < kWarps ? sh.wmax[lane] : 0u);
+    vmin = __reduce_min_sync(0xffffffffu, lane < kWarps ? sh.wmin[lane] : 0xffffffffu);
+    __syncthreads();
+    // ---- bisection: count(v >= lo) >= K > count(v >= hi), until few enough keys are at or above lo ------------------
+    const uint32_t slack = max(K >> 5, 8u);
+    uint32_t lo = vmin, n_lo = N;
+    unsigned long long hi = (unsigned long long)vmax + 1ull;      // (exclusive: no key is >= vmax + 1)
+#pragma unroll 1
+    while (hi - lo > 1ull && n_lo > K + slack) {
+        const uint32_t mid = (uint32_t)(lo + ((hi - lo) >> 1));
+        const uint32_t c = block_count([&](int x) { return v[x] >= mid; });      // (mid > 0: absent keys never count)
+        if (c >= K) { lo = mid; n_lo = c; } else hi = mid;
+    }
+    // more keys at or above lo than the list holds: they are exact ties at ord == lo (hi == lo + 1).  Take the keys
+    // above it and, of the tie, the K - count(v > lo) entries of lowest index (found by bisection on the index).
+    uint32_t tie_last = 0xffffffffu;                              // ties with index <= tie_last are kept
+    if (n_lo > (uint32_t)kWideCap) {
+        const uint32_t n_gt = block_count([&](int x) { return v[x] > lo; });
+        const uint32_t need = K - n_gt;                           // >= 1: count(v >= hi) < K
+        long long jl = -1, jh = (long long)N - 1;                 // count(idx <= jl) < need <= count(idx <= jh)
+#pragma unroll 1
+        while (jh - jl > 1) {
+            const long long jm = (jl + jh) >> 1;
+            const uint32_t c = block_count([&](int x) { return v[x] == lo && (long long)(x * kThreads + tid) <= jm; });
+            if (c >= need) jh = jm; else jl = jm;
+        }
+        tie_last = (uint32_t)jh;
+    }
+    // ---- gather the survivors (warp-aggregated reservation; the order in the list does not matter) -----------------
+#pragma unroll
+    for (int x = 0; x < kWideNV; ++x) {
+        const uint32_t idx = (uint32_t)(x * kThreads + tid);
+        const bool keep = v[x] != 0u && (v[x] > lo || (v[x] == lo && idx <= tie_last));
+        const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+        if (bal) {
+            uint32_t base = 0;
+            if (lane == 0) base = atomicAdd(&sh.cursor, (uint32_t)__popc(bal));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            const uint32_t pos = base + (uint32_t)__popc(bal & ((1u << lane) - 1u));
+            if (keep && pos < (uint32_t)kWideCap) ent[pos] = ((unsigned long long)(~v[x]) << 32) | idx;
+        }
+    }
+    __syncthreads();
+    const uint32_t n_s = min(sh.cursor, (uint32_t)kWideCap);      // K <= n_s (the min: memory safety on NaN-poisoned counts)
+    // ---- CTA s ranks its share of the survivors: a warp per entry, rank = number of smaller composites (all
+    // distinct).  The share is defined by the entry's INDEX (hashed, so that strided survivors still spread), not
+    // by its position: the lists of a user's CTAs hold the same set in different orders.
+    Out out;
+    out.score = out_score; out.parent = out_parent; out.code = out_code; out.row0 = (size_t)u * W_out;
+    // (R is a power of two; a warp looks at 32 entries at a time, one per lane, and then ranks the ones that are its
+    // CTA's, one after the other)
+#pragma unroll 1
+    for (uint32_t e0 = (uint32_t)warp * 32u; e0 < n_s; e0 += kWarps * 32u) {
+        const uint32_t e = e0 + lane;
+        const unsigned long long cand = e < n_s ? ent[e] : 0ull;
+        uint32_t todo = __ballot_sync(0xffffffffu, e < n_s && (int)((((uint32_t)cand * 2654435761u) >> 16) & (uint32_t)(R - 1)) == s);
+#pragma unroll 1
+        while (todo) {
+            const int src = __ffs(todo) - 1;
+            todo &= todo - 1u;
+            const unsigned long long c = __shfl_sync(0xffffffffu, cand, src);
+            uint32_t rk = 0;
+#pragma unroll 4
+            for (uint32_t i = lane; i < n_s; i += 32) rk += ent[i] < c ? 1u : 0u;
+            rk = __reduce_add_sync(0xffffffffu, rk);
+            if (lane == 0 && rk < K) out.put(ks, rk, c);
+        }
+    }
+}
+
 // per device: CTAs of topk_grid_kernel that can be co-resident (a cooperative launch must fit)
 int grid_capacity() {
     static PerDevice<int> cap;
@@ -868,6 +1004,27 @@ int launch_topk_grid(const float* logp, const float* score, int B, int W_in, int
     cfg.attrs = at; cfg.numAttrs = 1;
     STARK_CUDA_TRY(cudaLaunchKernelEx(&cfg, topk_grid_kernel, logp, score, W_in, C, c_shift, W_out, out_score,
                                       out_parent, out_code, S, G, state, pub, list, rel));
+    return STARK_OK;
+}
+
+// Wide selections over small candidate sets (topk_wide_kernel).  UNSUPPORTED = not served here.
+bool topk_wide_serves(long long N, int W_out) { return N <= kWideMaxN && W_out <= kWideMaxK; }
+
+int launch_topk_wide(const float* logp, const float* score, int B, int W_in, int C, int W_out, float* out_score,
+                     int32_t* out_parent, int32_t* out_code, cudaStream_t st) {
+    const long long N = (long long)W_in * C;
+    // measured (us per launch, here vs the cluster kernel): B = 8: 9.1-12.6 vs 13.9-14.4; B = 16: 11.3-12.6 vs 14.4;
+    // B = 32: 14.8 vs 13.6; B = 64: 19.2 vs 14.4 -- with few CTAs per user the ranking is no longer spread thin
+    if (!topk_wide_serves(N, W_out) || B > 16) return STARK_ERR_UNSUPPORTED;
+    int c_shift = -1;
+    if ((C & (C - 1)) == 0) { c_shift = 0; while ((1 << c_shift) < C) ++c_shift; }
+    // CTAs per user: enough that the ranking (n_s^2 compares per user) is spread thin, no more than two per SM in all
+    const int sms = num_sms() > 0 ? num_sms() : 148;
+    int R = 16;                                       // a power of two (the kernel masks a hash with R - 1)
+    while (R > 1 && R * B > sms) R >>= 1;             // (every CTA repeats the bisection: one CTA per SM at most)
+    topk_wide_kernel<<<dim3((unsigned)R, (unsigned)B), kThreads, 0, st>>>(logp, score, W_in, C, c_shift, W_out, out_score,
+                                                                         out_parent, out_code, R);
+    STARK_LAUNCH_CHECK();
     return STARK_OK;
 }
 

@@ -137,6 +137,33 @@ def test_mid_single_cta_path():
     _check(w, r.normal(0, 1, (1, 40)).astype(np.float32), 256)   # 201 finite keys + 55 of the -inf ties
 
 
+def test_wide_selection_over_small_candidate_sets():
+    """512 < N <= 8192 candidates per user and 256 < W_out <= 1024 (decode step 0 with a wide beam: PAPER.md:306,
+    512 of 8192 codes; config 4, 512 of 1024): R independent CTAs per user, bound by bisection, every CTA ranks a
+    slice (topk_wide_kernel).  Ragged N and C, W_out = N, many users (fewer CTAs each), ties by the thousand (the
+    second bisection, on the index), all keys equal, -inf blocks, signed zeros, the sizes just outside the path."""
+    r = _rng(11)
+    for (B, W_in, C, W_out) in [(8, 1, 1024, 512), (8, 1, 8192, 512), (1, 1, 8192, 1024), (3, 7, 333, 700),
+                               (2, 19, 27, 513), (2, 4, 256, 1024), (2, 1, 1000, 1000), (40, 1, 2048, 300),
+                               (300, 1, 600, 257), (2, 1, 8192, 1025), (2, 1, 8193, 512), (1, 3, 2731, 1024)]:
+        logits = r.normal(0, 2, (B, W_in, C))
+        logp = (logits - np.log(np.exp(logits).sum(-1, keepdims=True))).astype(np.float32)
+        score = None if W_in == 1 else np.sort(r.normal(-8, 2, (B, W_in)).astype(np.float32))[:, ::-1].copy()
+        _check(logp, score, W_out)
+        if B <= 8:
+            q = np.round(logp).astype(np.float32)                 # integer grid: ties in the thousands
+            _check(q, None if score is None else np.round(score).astype(np.float32), W_out)
+    _check(np.full((2, 4, 2048), -2.5, np.float32), None, 900)    # all equal: index order only
+    _check(np.full((1, 1, 8192), 0.0, np.float32), None, 1024)
+    z = np.zeros((2, 8, 512), np.float32); z[0, ::2] = -0.0; z[1, :, 3:] = -np.inf
+    _check(z, None, 400)
+    _check(z, np.zeros((2, 8), np.float32), 1024)
+    w = r.normal(-4, 1, (1, 10, 800)).astype(np.float32); w[0, :, 30:] = -np.inf; w[0, 9, 799] = 3.0
+    _check(w, r.normal(0, 1, (1, 10)).astype(np.float32), 512)   # 301 finite keys + 211 of the -inf ties
+    two = np.where(r.random((2, 1, 4096)) < 0.1, np.float32(-1.0), np.float32(-2.0)).astype(np.float32)
+    _check(two, None, 600)                                        # the boundary falls inside a huge tie
+
+
 @pytest.mark.parametrize("W_out", [1025, 1536, 2048, 3000])
 @pytest.mark.parametrize("B,W_in,C", [(2, 64, 1024), (1, 512, 1024), (1, 128, 8192), (3, 40, 1000)])
 def test_wide_outputs_above_1024(B, W_in, C, W_out):
