@@ -107,10 +107,15 @@ int plan_splits(const Dims& p, int dtype, int n_q, int max_len) {
 // Cluster size (= prefix splits) of the fused decode-attention kernel: 1, 2, 4 or 8.  Same cost model; the
 // exchange through distributed shared memory (~17 B/clk per SM) costs up to ~3.5 iterations when all 256
 // rows are live; resident CTAs: one per SM, whole clusters only (B200 co-schedules 15 clusters of 8).
-int plan_cluster_splits(const Dims& p, int n_q, int max_len) {
+// A RAGGED batch (prefix lengths differ: total_tokens < B * max_len) is not a sequence of equal waves: its CTAs are
+// handed out longest user first, so the launch takes about max(longest CTA, total work / resident CTAs).  (Measured at
+// config 5 step 0, lengths 1.2-8.2 K: the wave model chose 4 splits, 160 us; 1 split: see profiles.)
+int plan_cluster_splits(const Dims& p, int n_q, int max_len, int total_tokens) {
     const int sms = num_sms() > 0 ? num_sms() : 148;
     const int tiles = ceil_div(max_len, 128);
     const long long M = (long long)n_q * p.G;
+    const bool ragged = p.B >= 2 && (long long)max_len * p.B != (long long)total_tokens;
+    const double avg_tiles = (double)total_tokens / (128.0 * p.B);
     int best = 1;
     double best_cost = 1e300;
     for (int n = 1; n <= 8 && n <= tiles; n *= 2) {
@@ -119,7 +124,12 @@ int plan_cluster_splits(const Dims& p, int n_q, int max_len) {
         const int resident = n == 8 ? (sms / 8 - 3) * 8 : sms / n * n;
         const double iters = parity ? ceil_div(ceil_div(tiles, n), 2) + 0.5 : ceil_div(tiles, n);
         const double live = (double)(M < 256 ? M : 256) / 256.0;
-        const double cost = (double)ceil_div(ctas, resident > 0 ? resident : n) * (iters + 2.0) + (n > 1 ? 3.5 * live : 0.0);
+        double cost = (double)ceil_div(ctas, resident > 0 ? resident : n) * (iters + 2.0) + (n > 1 ? 3.5 * live : 0.0);
+        if (ragged) {
+            const double avg_iters = (parity ? 0.5 : 1.0) * avg_tiles / n;
+            const double fluid = (double)ctas * (avg_iters + 2.0) / (double)(resident > 0 ? resident : n);
+            cost = (fluid > iters + 2.0 ? fluid : iters + 2.0) + (n > 1 ? 3.5 * live : 0.0);
+        }
         if (cost < best_cost * 0.97) { best_cost = cost; best = n; }
     }
     return best;
@@ -232,7 +242,7 @@ int stark_decode_attn(const stark_shape_t* shape, const void* q, int n_q, int le
     if (rc != STARK_OK) return rc;
     const int32_t* anc_l = anc ? anc + (size_t)(level & 1) * p.B * p.Wmax * p.d : nullptr;
     return launch_decode_fused(p, q, n_q, level, k_prefix, v_prefix, cu_seqlens, total_tokens, max_prefix_len,
-                               plan_cluster_splits(p, n_q, max_prefix_len), k_suffix, v_suffix, anc_l, out,
+                               plan_cluster_splits(p, n_q, max_prefix_len, total_tokens), k_suffix, v_suffix, anc_l, out,
                                (cudaStream_t)stream);
 }
 
@@ -255,7 +265,7 @@ int stark_decode_step(const stark_shape_t* shape, const void* q, int n_q, int le
     const int32_t* anc_prev = level >= 1 ? anc + (size_t)((level - 1) & 1) * half : nullptr;
     int32_t* anc_new = (level >= 1 && write_anc) ? anc + (size_t)(level & 1) * half : nullptr;
     return launch_decode_fused(p, q, n_q, level, k_prefix, v_prefix, cu_seqlens, total_tokens, max_prefix_len,
-                               plan_cluster_splits(p, n_q, max_prefix_len), k_suffix, v_suffix, anc_prev, out,
+                               plan_cluster_splits(p, n_q, max_prefix_len, total_tokens), k_suffix, v_suffix, anc_prev, out,
                                (cudaStream_t)stream, level >= 1 ? k_new : nullptr, level >= 1 ? v_new : nullptr, parent,
                                anc_new);
 }
