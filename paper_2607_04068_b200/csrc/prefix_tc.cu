@@ -1176,10 +1176,14 @@ int launch_fused_d(const Dims& p, const CUtensorMap& tq, const CUtensorMap& tk, 
 }  // namespace
 
 // Parity mode (one Q tile per CTA, KV tiles alternating between the two accumulator sets) whenever its
-// doubled CTA count still fits the GPU in one wave; pair mode (K/V staged once per 256 rows) otherwise.
+// doubled CTA count still fits the GPU in one wave, and always for a single Q tile; pair mode (K/V staged once
+// per 256 rows) otherwise.
 bool prefix_tc_parity(const Dims& p, int n_q, int n_splits) {
     const int sms = num_sms() > 0 ? num_sms() : 148;
     const long long tiles_m = ((long long)n_q * p.G + BM - 1) / BM;
+    // a single Q tile (decode step 0 above all): pair mode would have the same CTA count and leave the second
+    // accumulator set idle -- every KV tile strictly after the other (config 3 step 0: 58 us for a 21 us stream)
+    if (tiles_m == 1) return true;
     return tiles_m * p.Hkv * p.B * n_splits <= sms;
 }
 
