@@ -17,9 +17,10 @@
 //      their K-th largest (K = W_out) as the user's bound L and releases the others: M disjoint groups, K of
 //      them with a key >= L, hence at least K keys >= L, hence the K-th best key is >= L and NO key below L can
 //      be selected.  With M ~ 4-8 K the number of keys >= L is 1.1-2 K.
-//   3. The rest of the slice is streamed ONCE against L (one fp32 add and one compare per key, 16-byte loads, 8
-//      per thread in flight); survivors (a handful per CTA) go to a shared-memory list, then the parked batch is
-//      filtered the same way.  Unsorted parents make L loose: when the list fills up, the CTA re-tightens its
+//   3. The parked batch is filtered against L (which frees the key cache), then the rest of the slice is streamed
+//      ONCE against L (one fp32 add and one compare per key): through a ring of 8 sixteen-byte slots per thread in
+//      the key cache, filled by cp.async, so that 7-8 loads of every thread are in flight all the time; survivors
+//      (a handful per CTA) go to a shared-memory list.  Unsorted parents make L loose: when the list fills up, the CTA re-tightens its
 //      own bound from the list (its K-th largest entry is again a valid bound) and compacts -- a streaming top-K.
 //   4. Every CTA writes its survivors, as composites (~ord(key) . index), and their count to its own segment of
 //      the user's list in the workspace and arrives at the user's second barrier.  Then EVERY CTA copies the
@@ -670,11 +671,35 @@ topk_grid_kernel(const float* __restrict__ logp, const float* __restrict__ score
     float thr = bound <= 0x007fffffu ? ninf : ord_inv(bound);     // (ord(-inf) = 0x007fffff; 0 = no bound)
     PROF(3);
 
-    // ---- 3. stream the rest of the slice once against the bound ---------------------------------------
+    // ---- 3. the rest of the slice, once, against the bound ---------------------------------------------------
     bool lost = false;                                   // survivors were dropped: the user takes the slow path
-    int since_check = 0;
-#pragma unroll 1
-    for (int k0 = kUnroll; k0 < my_chunks; k0 += kUnroll) {
+    // 3a. the parked batch first: that frees the key cache, of which a thread only ever touches its OWN 16-byte
+    // slots (8 of them), so no barrier is needed before it is reused as the ring of 3c
+#pragma unroll 2
+    for (int x = 0; x < kUnroll; ++x) {
+        const uint32_t i0 = x < my_chunks ? idx_of(x) : N;
+        if (i0 < N) {
+            const float4 k4 = *reinterpret_cast<const float4*>(cache + x * kChunk + tid * 4);
+            if (fmaxf(fmaxf(k4.x, k4.y), fmaxf(k4.z, k4.w)) >= thr) append4(sh, sv, thr, k4, i0);
+        }
+    }
+    // 3b. chunks kRing0 .. go through a ring of kUnroll slots per thread filled by cp.async: 7-8 loads of the thread
+    // are in flight ALL the time (batches held in registers went 8 -> 0 -> 8: one HBM round trip per batch, and
+    // the 64-register budget has no room for a second batch).  Primed here, under the batch that is already in
+    // registers (loaded across the barrier).
+    constexpr int kRing0 = 2 * kUnroll;
+    const uint32_t ring_base = (uint32_t)__cvta_generic_to_shared(cache) + (uint32_t)tid * 16u;
+    auto ring_issue = [&](int k) {                       // chunk k into slot k % kUnroll (always commits a group)
+        if (k < my_chunks) {
+            const uint32_t i0 = min(idx_of(k), N - 4);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(ring_base + (uint32_t)(k & (kUnroll - 1)) * (kChunk * 4u)),
+                         "l"(ks.lp + i0) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+#pragma unroll
+    for (int j = 0; j < kUnroll; ++j) ring_issue(kRing0 + j);
+    if (kUnroll < my_chunks) {
 #pragma unroll
         for (int x = 0; x < kUnroll; ++x) {
             if (ib[x] < N) {
@@ -684,10 +709,23 @@ topk_grid_kernel(const float* __restrict__ logp, const float* __restrict__ score
                 if (fmaxf(fmaxf(k4.x, k4.y), fmaxf(k4.z, k4.w)) >= thr) append4(sh, sv, thr, k4, ib[x]);   // rare
             }
         }
-        if (k0 + kUnroll < my_chunks) load_batch(k0 + kUnroll);
-        // the list is inspected every 4th batch only (a block barrier per batch would stop the warps from
+    }
+    // 3c. the ring
+    int since_check = 0;
+#pragma unroll 1
+    for (int k = kRing0; k < my_chunks; ++k) {
+        asm volatile("cp.async.wait_group %0;" ::"n"(kUnroll - 1) : "memory");   // chunk k has landed
+        const float4 v = *reinterpret_cast<const float4*>(cache + (k & (kUnroll - 1)) * kChunk + tid * 4);
+        ring_issue(k + kUnroll);                         // (its slot is free again)
+        const uint32_t i0 = idx_of(k);
+        if (i0 < N) {
+            const float sx = ks.score_of(ks.row_of(i0));
+            const float4 k4 = make_float4(__fadd_rn(sx, v.x), __fadd_rn(sx, v.y), __fadd_rn(sx, v.z), __fadd_rn(sx, v.w));
+            if (fmaxf(fmaxf(k4.x, k4.y), fmaxf(k4.z, k4.w)) >= thr) append4(sh, sv, thr, k4, i0);   // rare
+        }
+        // the list is inspected every 32 chunks only (a block barrier per batch would stop the warps from
         // overlapping each other's load latency)
-        if (++since_check < 4 && k0 + kUnroll < my_chunks) continue;
+        if (++since_check < 4 * kUnroll && k + 1 < my_chunks) continue;
         since_check = 0;
         __syncthreads();
         const uint32_t c1 = sh.sv_count;                 // (block-uniform)
@@ -698,18 +736,10 @@ topk_grid_kernel(const float* __restrict__ logp, const float* __restrict__ score
             thr = bound <= 0x007fffffu ? ninf : ord_inv(bound);
         }
     }
+    asm volatile("cp.async.wait_all;" ::: "memory");     // (nothing of the ring is in flight when the cache is reused)
     PROF(4);
-    // the parked batch against the (possibly tightened) bound
     uint32_t cnt = 0;
     if (!lost) {
-#pragma unroll 2
-        for (int x = 0; x < kUnroll; ++x) {
-            const uint32_t i0 = x < my_chunks ? idx_of(x) : N;
-            if (i0 < N) {
-                const float4 k4 = *reinterpret_cast<const float4*>(cache + x * kChunk + tid * 4);
-                if (fmaxf(fmaxf(k4.x, k4.y), fmaxf(k4.z, k4.w)) >= thr) append4(sh, sv, thr, k4, i0);
-            }
-        }
         __syncthreads();
         cnt = sh.sv_count;
         __syncthreads();
