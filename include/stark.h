@@ -283,7 +283,10 @@ int stark_beam_topk(const float* logp, const float* score_or_null, int B, int W_
  *   - ALL CALLS ON ONE GPU SHARE THE ARRAY: calls that may overlap on the GPU
  *     (streams without an ordering between them, several host threads) race
  *     and give undefined results.  Order them, or use stark_beam_topk with a
- *     workspace each.
+ *     workspace each;
+ *   - the first call on a device looks the array's address up
+ *     (cudaGetSymbolAddress): make it outside stream capture; every later call
+ *     may be captured into a CUDA graph.
  * logp, score_or_null, out_*: device pointers, as for stark_beam_topk.
  * Errors: INVALID_ARG as stark_beam_topk, WORKSPACE (beyond the static
  * maximum), UNSUPPORTED (not an sm_100 device), CUDA.

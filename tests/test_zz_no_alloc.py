@@ -71,6 +71,32 @@ def test_static_scratch_matches_oracle():
         assert np.array_equal(s_g[u].view(np.uint32), s_r.view(np.uint32))
 
 
+def test_static_scratch_under_graph_capture():
+    """The use case the entry point exists for: captured into a CUDA graph (no allocation may happen there) and
+    replayed.  The first call per device resolves the array's address and is made eagerly, before the capture."""
+    import torch
+    from paper_2607_04068_b200.decode import beam_topk, beam_topk_static
+    B, W_in, C, W_out = 2, 256, 1024, 256
+    logp, score = _inputs(B, W_in, C, 7)
+    lp, sc = torch.from_numpy(logp).cuda(), torch.from_numpy(score).cuda()
+    out = _outs(B, W_out)
+    beam_topk_static(lp, sc, W_out, out)                     # eager warm-up
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        beam_topk_static(lp, sc, W_out, out)
+    for rep in range(2):
+        logp, score = _inputs(B, W_in, C, 70 + rep)          # new contents in the captured buffers
+        lp.copy_(torch.from_numpy(logp)); sc.copy_(torch.from_numpy(score))
+        for o in out:
+            o.fill_(-1)
+        g.replay()
+        torch.cuda.synchronize()
+        ref = beam_topk(lp, sc, W_out)
+        for a, b in zip(out, ref):
+            assert torch.equal(a.view(torch.int32), b.view(torch.int32)), f"replay {rep}"
+
+
 def test_beyond_the_static_maximum_is_rejected():
     """64 users x 131 072 candidates need 10.5 MB of workspace: more than the 9 MiB array.  Clear error, nothing
     launched, outputs untouched; the workspace path serves the same problem."""
